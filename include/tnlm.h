@@ -1,0 +1,135 @@
+/*
+ * tnlm.h -- C ABI of libtnlm: the data-parallel hot path of
+ * "Low-dose 4DCT Reconstruction via Temporal Nonlocal Means" (arxiv 1009.1351) on one
+ * NVIDIA B200 (sm_100a).  Citations are PAPER.md:L<line>.
+ *
+ * One modified forward-backward-splitting iteration over all N respiratory phases of a CT
+ * slice at once ("TNLM Algorithm"):
+ *     g^(k) = CGLS_{M1}( f^(k-1) ; P, P^T, Sigma^-1, y )               step 2   (L103-L135)
+ *     w     = TNLM weights of g^(k) to the two cyclic neighbour phases  step 3   (Eq. 8)
+ *     f^(k) = max( GaussJacobi_{M2}( g^(k) ; w, mu ), 0 )               steps 4-5 (Eq. 7)
+ *
+ * Conventions
+ *   N = n_phase, image ny x nx (row-major), S = n_slices independent slices.
+ *   Pixel (r,c) is the square of side pixel_mm centred at
+ *       X = (c-(nx-1)/2)*pixel_mm,  Y = (r-(ny-1)/2)*pixel_mm           (isocentre = grid centre).
+ *   Fan beam, equiangular arc detector (L212).  View angle th: source S = sid*(cos th, sin th);
+ *   bin k sits at fan angle gam_k = (k-(n_bins-1)/2+bin_offset)*bin_pitch/sdd; its pencil ray
+ *   leaves S in direction -(cos(th+gam_k), sin(th+gam_k)).
+ *   (P f)[v,k] = sum_pix length(ray_{v,k} ∩ pixel) * f[pix]   (radiological path, Siddon, L212);
+ *   P^T is its exact matrix transpose (L79).  A ray lying exactly on a grid line is attributed
+ *   to the pixel on its upper side.
+ *   TNLM: window W x W (odd, a=(W-1)/2), patch d x d (odd, b=(d-1)/2).  Patches are extended by
+ *   zero outside the image; candidates y = x+delta, delta in [-a,a]^2, outside the image are
+ *   excluded from the sums and from Z.  Phases are cyclic: f_{N+1} = f_1 (L81).
+ *       D(x,delta)   = sum_{p in [-b,b]^2} ( g_i(x+p) - g_j(x+delta+p) )^2               (L90)
+ *       w_ij(x,x+delta) = exp(-D/h^2) / Z,  Z = sum over in-image delta               (Eq. 3/8, L94)
+ *       u_i' (x) = g_i(x)/(1+mu) + mu/(2mu+2) * sum_{j=i-1,i+1} sum_delta w_ij u_j(x+delta)  (Eq. 7)
+ *   `mu` is the paper's mu-hat = mu/beta (L141).  The softmax is evaluated in a shifted,
+ *   overflow/underflow-safe form; the value is the one defined above.
+ *
+ * Memory
+ *   Every `float *` of the device entry points is a DEVICE pointer to a caller-owned,
+ *   contiguous fp32 buffer:  images [S][N][ny][nx],  sinograms / weights [S][N][V][B].
+ *   The `_host` entry points take HOST pointers with the same layouts.  The library never
+ *   frees or keeps caller buffers.  Inputs are never modified.  Outputs may alias the input
+ *   image of the same call where stated.  Workspace is owned by the handle, grown lazily to the
+ *   largest n_slices seen, and freed by tnlm_destroy.
+ *
+ * Execution
+ *   Device entry points enqueue work on `stream` (a cudaStream_t passed as void*, NULL = the
+ *   legacy default stream) and return without synchronising; all scalars of CGLS stay on the
+ *   device.  `_host` entry points copy in, run, copy out and synchronise `stream` before
+ *   returning.  A handle must not be used from two streams or threads at once.
+ *
+ * Errors
+ *   Every call returns a tnlm_status; nothing throws, exits or falls back to the CPU.
+ *   tnlm_last_error(handle) gives a handle-owned message for the last failing call.
+ */
+#ifndef TNLM_H
+#define TNLM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TNLM_OK = 0,
+    TNLM_INVALID_ARG = 1, /* NULL handle/buffer, bad sizes, even/too small window or patch, h<=0,
+                             mu<0, negative iteration counts, projector call without geometry,
+                             sid>=sdd, image not strictly inside the source circle */
+    TNLM_CUDA_ERROR = 2,  /* a CUDA runtime call failed; message from cudaGetErrorString */
+    TNLM_ALLOC_FAILED = 3,
+    TNLM_UNSUPPORTED = 4  /* device is not sm_100, patch/window above the compiled maximum
+                             (patch <= 9, window <= 31), flat detector */
+} tnlm_status;
+
+typedef struct tnlm_handle tnlm_handle; /* opaque: geometry tables + workspace */
+
+/* Scan geometry of one slice.  Read once by tnlm_create; not kept. */
+typedef struct {
+    int n_views;              /* views per phase, V */
+    int n_bins;               /* detector bins, B */
+    double sid_mm;            /* source to rotation centre */
+    double sdd_mm;            /* source to detector */
+    double bin_pitch_mm;      /* bin spacing along the arc */
+    double bin_offset;        /* detector shift in bins, 0 = centred */
+    double pixel_mm;          /* square pixel side */
+    int detector_arc;         /* 1 = equiangular arc (the paper's); 0 = flat -> TNLM_UNSUPPORTED */
+    const double *angles_rad; /* HOST, [n_phase][n_views] source angles; P_i differs per phase (L75) */
+} tnlm_geometry;
+
+/* Create a handle.  `geometry` may be NULL: TNLM-only handle, projector/CGLS/reconstruct
+ * calls then return TNLM_INVALID_ARG.  window/patch odd >= 1; h > 0 finite; mu >= 0. */
+int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_phase, int window, int patch,
+                float h, float mu, tnlm_handle **out);
+int tnlm_destroy(tnlm_handle *handle);
+
+/* sino = P img.  img [S][N][ny][nx] -> sino [S][N][V][B]; must not alias. */
+int tnlm_project(tnlm_handle *handle, const float *img, float *sino, int n_slices, void *stream);
+
+/* img = P^T sino, the exact transpose of tnlm_project; must not alias. */
+int tnlm_backproject(tnlm_handle *handle, const float *sino, float *img, int n_slices, void *stream);
+
+/* "CGLS Algorithm": m1 steps on P_n = Sigma^-1/2 P, y_n = Sigma^-1/2 y,
+ * per phase and slice, warm-started at f_in; g_out = u^(m1).  w = diagonal of Sigma^-1
+ * (NULL = identity).  No positivity clip.  m1 = 0 copies f_in.  If ||P_n s||^2 or
+ * ||P_n^T r||^2 is 0 for a phase that phase stops and keeps its iterate (no NaN).
+ * g_out may alias f_in. */
+int tnlm_cgls_step(tnlm_handle *handle, const float *f_in, const float *y, const float *w, int m1,
+                   float *g_out, int n_slices, void *stream);
+
+/* Steps 3-5: weights from g (Eq. 8), m2 Gauss-Jacobi sweeps of Eq. (7)
+ * from u^0 = g with the weights fixed, then f = max(u, 0) once.  m2 = 0 gives max(g, 0).
+ * f_out may alias g. */
+int tnlm_regularize_step(tnlm_handle *handle, const float *g, int m2, float *f_out, int n_slices,
+                         void *stream);
+
+/* "TNLM Algorithm": f^0 = f0 (NULL = zeros; the paper's FBP start is the
+ * caller's to supply), k_outer times { cgls_step(m1) ; regularize_step(m2) }.  k_outer = 0
+ * copies f0.  f_out may alias f0. */
+int tnlm_reconstruct(tnlm_handle *handle, const float *y, const float *w, const float *f0,
+                     int k_outer, int m1, int m2, float *f_out, int n_slices, void *stream);
+
+/* Same operations with HOST buffers: host->device copies, the device path above, the
+ * device->host copy of the result, and a stream synchronise, all inside the call. */
+int tnlm_regularize_step_host(tnlm_handle *handle, const float *g_host, int m2, float *f_out_host,
+                              int n_slices, void *stream);
+int tnlm_reconstruct_host(tnlm_handle *handle, const float *y_host, const float *w_host,
+                          const float *f0_host, int k_outer, int m1, int m2, float *f_out_host,
+                          int n_slices, void *stream);
+
+/* Message of the last failing call on this handle ("" if none); handle-owned, valid until the
+ * next call on the handle.  NULL handle -> message of the last failed tnlm_create. */
+const char *tnlm_last_error(const tnlm_handle *handle);
+
+/* Number of CUDA kernels this handle has launched so far (for benchmark bookkeeping). */
+long long tnlm_launch_count(const tnlm_handle *handle);
+
+/* Library version string, e.g. "tnlm-b200 0.1 (sm_100a)". */
+const char *tnlm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TNLM_H */

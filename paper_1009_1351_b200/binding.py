@@ -1,0 +1,202 @@
+"""ctypes binding of libtnlm.so: same names as include/tnlm.h, argument marshalling only."""
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+STATUS = {0: "TNLM_OK", 1: "TNLM_INVALID_ARG", 2: "TNLM_CUDA_ERROR", 3: "TNLM_ALLOC_FAILED", 4: "TNLM_UNSUPPORTED"}
+
+# every symbol include/tnlm.h declares
+EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "tnlm_cgls_step",
+           "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
+           "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version"]
+
+
+class TnlmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class _CGeometry(C.Structure):
+    _fields_ = [("n_views", C.c_int), ("n_bins", C.c_int), ("sid_mm", C.c_double), ("sdd_mm", C.c_double),
+                ("bin_pitch_mm", C.c_double), ("bin_offset", C.c_double), ("pixel_mm", C.c_double),
+                ("detector_arc", C.c_int), ("angles_rad", C.POINTER(C.c_double))]
+
+
+@dataclass
+class Geometry:
+    """Fan-beam arc-detector geometry of one slice; angles_rad is [n_phase][n_views]."""
+    n_views: int
+    n_bins: int
+    sid_mm: float
+    sdd_mm: float
+    bin_pitch_mm: float
+    angles_rad: np.ndarray
+    bin_offset: float = 0.0
+    pixel_mm: float = 1.0
+    detector_arc: int = 1
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libtnlm.so")
+
+
+def library():
+    """Load libtnlm.so (never builds, never falls back)."""
+    global _LIB
+    if _LIB is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: run `python -m paper_1009_1351_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        P, I, F = C.c_void_p, C.c_int, C.c_float
+        L.tnlm_create.argtypes = [C.POINTER(_CGeometry), I, I, I, I, I, F, F, C.POINTER(P)]
+        L.tnlm_destroy.argtypes = [P]
+        L.tnlm_project.argtypes = [P, P, P, I, P]
+        L.tnlm_backproject.argtypes = [P, P, P, I, P]
+        L.tnlm_cgls_step.argtypes = [P, P, P, P, I, P, I, P]
+        L.tnlm_regularize_step.argtypes = [P, P, I, P, I, P]
+        L.tnlm_reconstruct.argtypes = [P, P, P, P, I, I, I, P, I, P]
+        L.tnlm_regularize_step_host.argtypes = [P, P, I, P, I, P]
+        L.tnlm_reconstruct_host.argtypes = [P, P, P, P, I, I, I, P, I, P]
+        L.tnlm_last_error.argtypes = [P]
+        L.tnlm_last_error.restype = C.c_char_p
+        L.tnlm_launch_count.argtypes = [P]
+        L.tnlm_launch_count.restype = C.c_longlong
+        L.tnlm_version.restype = C.c_char_p
+        _LIB = L
+    return _LIB
+
+
+def version() -> str:
+    return library().tnlm_version().decode()
+
+
+class Handle:
+    """Owner of a tnlm_handle*; destroyed with the object."""
+
+    def __init__(self, ptr, nx, ny, n_phase, geometry):
+        self.ptr, self.nx, self.ny, self.n_phase, self.geometry = ptr, nx, ny, n_phase, geometry
+
+    def close(self):
+        if self.ptr:
+            library().tnlm_destroy(self.ptr)
+            self.ptr = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launch_count(self) -> int:
+        return int(library().tnlm_launch_count(self.ptr))
+
+    def check(self, rc):
+        if rc != 0:
+            raise TnlmError(rc, (library().tnlm_last_error(self.ptr) or b"").decode())
+
+
+def create(geometry, nx, ny, n_phase, window, patch, h, mu) -> Handle:
+    """tnlm_create: geometry may be None (TNLM-only handle)."""
+    L = library()
+    out = C.c_void_p()
+    if geometry is None:
+        rc = L.tnlm_create(None, nx, ny, n_phase, window, patch, h, mu, C.byref(out))
+    else:
+        ang = np.ascontiguousarray(geometry.angles_rad, dtype=np.float64)
+        if ang.shape != (n_phase, geometry.n_views):
+            raise ValueError(f"angles_rad must be [n_phase][n_views], got {ang.shape}")
+        cg = _CGeometry(geometry.n_views, geometry.n_bins, geometry.sid_mm, geometry.sdd_mm,
+                        geometry.bin_pitch_mm, geometry.bin_offset, geometry.pixel_mm,
+                        geometry.detector_arc, ang.ctypes.data_as(C.POINTER(C.c_double)))
+        rc = L.tnlm_create(C.byref(cg), nx, ny, n_phase, window, patch, h, mu, C.byref(out))
+    if rc != 0:
+        raise TnlmError(rc, (L.tnlm_last_error(None) or b"").decode())
+    return Handle(out.value, nx, ny, n_phase, geometry)
+
+
+# ---- device-pointer calls: torch tensors provide memory and the current stream -----------------
+def _dev(t, name):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+
+
+def _slices(h: Handle, t, per_slice):
+    n = t.numel()
+    if n % per_slice:
+        raise ValueError("tensor size is not a whole number of slices")
+    return n // per_slice
+
+
+def project(h: Handle, img, sino, stream=None):
+    S = _slices(h, img, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_project(h.ptr, _dev(img, "img"), _dev(sino, "sino"), S, _stream(stream)))
+    return sino
+
+
+def backproject(h: Handle, sino, img, stream=None):
+    S = _slices(h, img, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_backproject(h.ptr, _dev(sino, "sino"), _dev(img, "img"), S, _stream(stream)))
+    return img
+
+
+def cgls_step(h: Handle, f_in, y, w, m1, g_out, stream=None):
+    S = _slices(h, f_in, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_cgls_step(h.ptr, _dev(f_in, "f_in"), _dev(y, "y"), _dev(w, "w"), m1,
+                                     _dev(g_out, "g_out"), S, _stream(stream)))
+    return g_out
+
+
+def regularize_step(h: Handle, g, m2, f_out, stream=None):
+    S = _slices(h, g, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_regularize_step(h.ptr, _dev(g, "g"), m2, _dev(f_out, "f_out"), S, _stream(stream)))
+    return f_out
+
+
+def reconstruct(h: Handle, y, w, f0, k_outer, m1, m2, f_out, stream=None):
+    S = _slices(h, f_out, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_reconstruct(h.ptr, _dev(y, "y"), _dev(w, "w"), _dev(f0, "f0"), k_outer, m1, m2,
+                                       _dev(f_out, "f_out"), S, _stream(stream)))
+    return f_out
+
+
+# ---- host-pointer calls: CPU tensors (pinned or pageable); copies happen inside the library ----
+def _host(t, name):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float32 CPU tensor")
+    return t.data_ptr()
+
+
+def regularize_step_host(h: Handle, g_host, m2, f_out_host, stream=None):
+    S = _slices(h, g_host, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_regularize_step_host(h.ptr, _host(g_host, "g_host"), m2,
+                                                _host(f_out_host, "f_out_host"), S, _stream(stream)))
+    return f_out_host
+
+
+def reconstruct_host(h: Handle, y_host, w_host, f0_host, k_outer, m1, m2, f_out_host, stream=None):
+    S = _slices(h, f_out_host, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_reconstruct_host(h.ptr, _host(y_host, "y_host"), _host(w_host, "w_host"),
+                                            _host(f0_host, "f0_host"), k_outer, m1, m2,
+                                            _host(f_out_host, "f_out_host"), S, _stream(stream)))
+    return f_out_host

@@ -1,0 +1,344 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle.
+
+All tests need a B200: `pytest -m gpu`.  Bars (BASELINE.json north_star): relative L2 <= 1e-4
+per single step, <= 1e-3 after 20 outer iterations, adjoint identity ~1e-5 relative, fp32.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+STEP_TOL = 1e-4
+RECON_TOL = 1e-3
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def T():
+    import torch
+    import paper_1009_1351_b200 as tn
+    assert torch.cuda.is_available()
+    return torch, tn
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def handles(tn, cfg, geom=True, **over):
+    kw = workloads.geometry_kwargs(cfg)
+    g = tn.Geometry(**kw) if geom and cfg.V > 0 else None
+    og = oracle.Geometry(**kw) if geom and cfg.V > 0 else None
+    h = tn.create(g, cfg.L, cfg.L, cfg.N, over.get("window", cfg.window), over.get("patch", cfg.patch),
+                  over.get("h", cfg.h), over.get("mu", cfg.mu))
+    return h, og
+
+
+# ------------------------------------------------------------------------------- projectors
+def small_geom_cfg(L=48, N=3, V=40, B=80):
+    return workloads.Config("small", L=L, N=N, V=V, B=B, pitch=1.0, sid=90.0, sdd=150.0, I0=1e4,
+                            window=5, patch=3, h=0.01, mu=0.1)
+
+
+@pytest.mark.parametrize("cfg", [workloads.config(1), small_geom_cfg(), small_geom_cfg(L=37, N=2, V=23, B=61)],
+                         ids=["cfg1", "small48", "odd37"])
+def test_project_and_backproject_match_oracle(T, cfg):
+    torch, tn = T
+    h, og = handles(tn, cfg)
+    rng = np.random.default_rng(7)
+    ph = workloads.make_inputs(cfg)["phantom"][0]
+    for img in (ph, rng.random(ph.shape) * 0.02):
+        sino = torch.empty(cfg.N, cfg.V, cfg.B, device="cuda")
+        tn.project(h, dev(torch, img), sino)
+        want = oracle.project(og, img.astype(np.float32))
+        assert rel(sino.cpu().numpy(), want) < STEP_TOL
+    s = rng.random((cfg.N, cfg.V, cfg.B))
+    out = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.backproject(h, dev(torch, s), out)
+    want = oracle.backproject(og, s.astype(np.float32), cfg.L, cfg.L)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+
+
+def test_adjoint_identity_on_gpu(T):
+    torch, tn = T
+    cfg = workloads.config(1)
+    h, _ = handles(tn, cfg)
+    g = torch.Generator(device="cuda").manual_seed(3)
+    f = torch.randn(cfg.N, cfg.L, cfg.L, device="cuda", generator=g)
+    s = torch.randn(cfg.N, cfg.V, cfg.B, device="cuda", generator=g)
+    Pf = torch.empty_like(s); Pts = torch.empty_like(f)
+    tn.project(h, f, Pf); tn.backproject(h, s, Pts)
+    lhs = (Pf.double() * s.double()).sum().item(); rhs = (f.double() * Pts.double()).sum().item()
+    scale = (Pf.double().norm() * s.double().norm()).item()
+    assert abs(lhs - rhs) <= 1e-5 * scale, (lhs, rhs, scale)
+    # positive data (no cancellation in the inner product): relative to the value itself
+    f.abs_(); s.abs_()
+    tn.project(h, f, Pf); tn.backproject(h, s, Pts)
+    lhs = (Pf.double() * s.double()).sum().item(); rhs = (f.double() * Pts.double()).sum().item()
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
+
+
+def test_gpu_projector_matrix_is_exactly_symmetric_entrywise(T):
+    # P^T built row by row from tnlm_backproject equals P built column by column from tnlm_project,
+    # bit for bit (both kernels evaluate the same per-(ray,pixel) length).
+    torch, tn = T
+    cfg = workloads.Config("tiny", L=6, N=1, V=5, B=14, pitch=1.0, sid=20.0, sdd=35.0, window=3, patch=3)
+    h, og = handles(tn, cfg)
+    npx, nr = cfg.L * cfg.L, cfg.V * cfg.B
+    cols = torch.empty(npx, nr, device="cuda"); rows = torch.empty(nr, npx, device="cuda")
+    for p in range(npx):
+        e = torch.zeros(npx, device="cuda"); e[p] = 1.0
+        tn.project(h, e.view(1, cfg.L, cfg.L).contiguous(), cols[p].view(1, cfg.V, cfg.B))
+    for q in range(nr):
+        e = torch.zeros(nr, device="cuda"); e[q] = 1.0
+        tn.backproject(h, e.view(1, cfg.V, cfg.B).contiguous(), rows[q].view(1, cfg.L, cfg.L))
+    assert torch.equal(cols.t().contiguous(), rows)
+    # and it is the oracle's matrix
+    A = np.stack([oracle.project(og, np.eye(npx)[p].reshape(1, cfg.L, cfg.L)).ravel() for p in range(npx)], axis=1)
+    assert np.abs(rows.cpu().numpy() - A).max() < 2e-5
+
+
+def test_full_size_projectors_on_sampled_outputs(T):
+    # BASELINE config 4 geometry (512^2, 60 views, 888 bins), launch configuration of the bench;
+    # the oracle computes sampled rays / pixels one by one.
+    torch, tn = T
+    cfg = workloads.config(4)
+    h, og = handles(tn, cfg)
+    rng = np.random.default_rng(11)
+    ph = workloads.make_inputs(cfg)["phantom"][0]
+    img = ph + 0.001 * rng.standard_normal(ph.shape)
+    sino = torch.empty(cfg.N, cfg.V, cfg.B, device="cuda")
+    tn.project(h, dev(torch, img), sino)
+    rays = rng.integers(0, cfg.N * cfg.V * cfg.B, 3000)
+    want = oracle.project_rays(og, img.astype(np.float32), rays)
+    assert rel(sino.cpu().numpy().ravel()[rays], want) < STEP_TOL
+    s = rng.random((cfg.N, cfg.V, cfg.B))
+    out = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.backproject(h, dev(torch, s), out)
+    pix = rng.integers(0, cfg.N * cfg.L * cfg.L, 400)
+    want = oracle.backproject_pixels(og, s.astype(np.float32), cfg.L, cfg.L, pix)
+    assert rel(out.cpu().numpy().ravel()[pix], want) < STEP_TOL
+
+
+# ------------------------------------------------------------------------------------- CGLS
+@pytest.mark.parametrize("m1", [0, 1, 3, 5])
+def test_cgls_step_matches_oracle(T, m1):
+    torch, tn = T
+    cfg = workloads.config(1)
+    inp = workloads.make_inputs(cfg)
+    h, og = handles(tn, cfg)
+    y, w = inp["y"][0].astype(np.float32), inp["w"][0].astype(np.float32)
+    f_in = (inp["phantom"][0] * 0.5).astype(np.float32)
+    g = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.cgls_step(h, dev(torch, f_in), dev(torch, y), dev(torch, w), m1, g)
+    want = oracle.cgls_step(og, f_in, y, w, m1)
+    assert rel(g.cpu().numpy(), want) < STEP_TOL
+    # unweighted (w = NULL), in place
+    f = dev(torch, f_in)
+    tn.cgls_step(h, f, dev(torch, y), None, m1, f)
+    assert rel(f.cpu().numpy(), oracle.cgls_step(og, f_in, y, None, m1)) < STEP_TOL
+
+
+def test_cgls_zero_data_breakdown_keeps_iterate(T):
+    torch, tn = T
+    cfg = workloads.config(1)
+    h, _ = handles(tn, cfg)
+    z = torch.zeros(cfg.N, cfg.L, cfg.L, device="cuda")
+    y = torch.zeros(cfg.N, cfg.V, cfg.B, device="cuda")
+    g = torch.full_like(z, 7.0)
+    tn.cgls_step(h, z, y, None, 3, g)
+    assert torch.equal(g, z)
+
+
+# ------------------------------------------------------------------------------------- TNLM
+def noisy_stack(N, ny, nx, seed, sigma=0.002):
+    cfg = workloads.Config("p", L=max(ny, nx), N=N)
+    ph = workloads.make_inputs(cfg)["phantom"][0][:, :ny, :nx]
+    return (ph + sigma * np.random.default_rng(seed).standard_normal(ph.shape)).astype(np.float32)
+
+
+@pytest.mark.parametrize("N,ny,nx,W,d,h,mu,m2", [
+    (3, 40, 70, 5, 3, 0.01, 0.1, 1),       # one CTA tile + ragged tails
+    (10, 64, 64, 5, 3, 0.01, 0.1, 1),      # config 1 shape
+    (4, 100, 130, 11, 5, 0.008, 0.1, 2),   # several tiles, interior and border, config 2/3 window
+    (3, 97, 150, 15, 7, 0.005, 0.2, 1),    # config 4/5 window
+    (2, 33, 65, 7, 1, 0.004, 0.5, 3),      # N=2: both neighbours are the same phase; patch 1
+    (1, 50, 50, 3, 9, 0.02, 0.3, 2),       # N=1 degenerate self-NLM; patch 9
+    (5, 30, 30, 1, 3, 0.01, 0.4, 2),       # window 1
+])
+def test_regularize_step_matches_oracle(T, N, ny, nx, W, d, h, mu, m2):
+    torch, tn = T
+    g = noisy_stack(N, ny, nx, seed=N * 100 + W)
+    g[0, 3, 4] = -0.003
+    hd = tn.create(None, nx, ny, N, W, d, h, mu)
+    out = torch.empty(N, ny, nx, device="cuda")
+    tn.regularize_step(hd, dev(torch, g), m2, out)
+    want = oracle.regularize_step(g, W, d, h, mu, m2)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+    assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
+
+
+def test_regularize_edge_cases(T):
+    torch, tn = T
+    N, ny, nx = 3, 45, 77
+    g = noisy_stack(N, ny, nx, 5) - 0.001
+    gd = dev(torch, g)
+    # m2 = 0 -> max(g,0) bit-exact; mu = 0 -> same
+    h0 = tn.create(None, nx, ny, N, 5, 3, 0.01, 0.3)
+    out = torch.empty_like(gd)
+    tn.regularize_step(h0, gd, 0, out)
+    assert torch.equal(out, gd.clamp_min(0))
+    hmu0 = tn.create(None, nx, ny, N, 5, 3, 0.01, 0.0)
+    tn.regularize_step(hmu0, gd, 2, out)
+    assert torch.equal(out, gd.clamp_min(0))
+    # in place (f_out aliases g) equals out of place
+    a = torch.empty_like(gd); tn.regularize_step(h0, gd, 2, a)
+    b = gd.clone(); tn.regularize_step(h0, b, 2, b)
+    assert torch.equal(a, b)
+    # tiny h: every D/h^2 is huge -> the shifted softmax must not underflow (oracle agrees)
+    g1 = np.random.default_rng(2).random((N, ny, nx)).astype(np.float32)
+    ht = tn.create(None, nx, ny, N, 5, 3, 1e-3, 0.5)
+    tn.regularize_step(ht, dev(torch, g1), 1, out)
+    assert torch.isfinite(out).all()
+    assert rel(out.cpu().numpy(), oracle.regularize_step(g1, 5, 3, 1e-3, 0.5, 1)) < STEP_TOL
+    # huge h: box mean
+    hh = tn.create(None, nx, ny, N, 5, 3, 1e6, 0.5)
+    tn.regularize_step(hh, dev(torch, g1), 1, out)
+    assert rel(out.cpu().numpy(), oracle.regularize_step(g1, 5, 3, 1e6, 0.5, 1)) < STEP_TOL
+    # constant image is a fixed point
+    cst = torch.full((N, ny, nx), 0.0173, device="cuda")
+    tn.regularize_step(h0, cst, 3, out)
+    assert (out - cst).abs().max().item() < 1e-8
+
+
+def test_regularize_multi_slice_equals_per_slice(T):
+    torch, tn = T
+    N, ny, nx, S = 3, 40, 72, 3
+    g = np.stack([noisy_stack(N, ny, nx, 20 + s) for s in range(S)])
+    hd = tn.create(None, nx, ny, N, 7, 5, 0.008, 0.2)
+    out = torch.empty(S, N, ny, nx, device="cuda")
+    tn.regularize_step(hd, dev(torch, g), 2, out)
+    for s in range(S):
+        one = torch.empty(N, ny, nx, device="cuda")
+        tn.regularize_step(hd, dev(torch, g[s]), 2, one)
+        assert torch.equal(out[s], one)
+
+
+def test_config2_full_size_on_sampled_pixels(T):
+    # BASELINE config 2 (256^2 x 10, W=11, d=5, h=0.008, 10 sweeps) in the bench's launch
+    # configuration; sampled pixels of sweep 1 against the oracle's one-pixel evaluation, plus the
+    # full 2-sweep result (the clip acts only after the last sweep, so u^(1) inside is unclipped).
+    torch, tn = T
+    cfg = workloads.config(2)
+    g = workloads.make_inputs(cfg)["g"][0].astype(np.float32)
+    hd, _ = handles(tn, cfg)
+    gd = dev(torch, g)
+    u1 = torch.empty_like(gd); u2 = torch.empty_like(gd)
+    tn.regularize_step(hd, gd, 1, u1)
+    tn.regularize_step(hd, gd, 2, u2)
+    pix = np.random.default_rng(0).integers(0, g.size, 4000)
+    want1 = oracle.gj_sweep_pixels(g, g, cfg.window, cfg.patch, cfg.h, cfg.mu, pix)
+    assert rel(u1.cpu().numpy().ravel()[pix], np.maximum(want1, 0)) < STEP_TOL
+    full = oracle.regularize_step(g, cfg.window, cfg.patch, cfg.h, cfg.mu, 2)
+    assert rel(u2.cpu().numpy(), full) < STEP_TOL
+    # 10 sweeps: finite, non-negative, and a contraction towards a fixed point
+    u10 = torch.empty_like(gd); u9 = torch.empty_like(gd)
+    tn.regularize_step(hd, gd, 10, u10); tn.regularize_step(hd, gd, 9, u9)
+    assert torch.isfinite(u10).all() and (u10 >= 0).all()
+    assert (u10 - u9).abs().max().item() < (u2 - u1).abs().max().item()
+
+
+def test_config4_window_full_size_on_sampled_pixels(T):
+    torch, tn = T
+    cfg = workloads.config(4)
+    ph = workloads.make_inputs(workloads.Config("p", L=512, N=10))["phantom"][0]
+    g = (ph + 0.002 * np.random.default_rng(9).standard_normal(ph.shape)).astype(np.float32)
+    hd = tn.create(None, 512, 512, 10, cfg.window, cfg.patch, cfg.h, cfg.mu)
+    out = torch.empty(10, 512, 512, device="cuda")
+    tn.regularize_step(hd, dev(torch, g), 1, out)
+    rng = np.random.default_rng(1)
+    pix = np.concatenate([rng.integers(0, g.size, 1500),
+                          np.array([0, 511, 512 * 511, 512 * 512 - 1, 5 * 512 * 512 + 7 * 512 + 3])])
+    want = oracle.gj_sweep_pixels(g, g, cfg.window, cfg.patch, cfg.h, cfg.mu, pix)
+    assert rel(out.cpu().numpy().ravel()[pix], np.maximum(want, 0)) < STEP_TOL
+
+
+# ------------------------------------------------------------------------------ whole iteration
+def test_reconstruct_config1_matches_oracle(T):
+    torch, tn = T
+    cfg = workloads.config(1)
+    inp = workloads.make_inputs(cfg)
+    h, og = handles(tn, cfg)
+    y, w = inp["y"][0].astype(np.float32), inp["w"][0].astype(np.float32)
+    out = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), None, cfg.K, cfg.m1, cfg.m2, out)
+    want = oracle.reconstruct(og, y, w, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, cfg.K, cfg.m1, cfg.m2)
+    assert rel(out.cpu().numpy(), want) < RECON_TOL
+    # k = 0 copies f0; one outer iteration = cgls_step then regularize_step
+    f0 = dev(torch, inp["phantom"][0])
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), f0, 0, 3, 1, out)
+    assert torch.equal(out, f0)
+    g = torch.empty_like(out); f1 = torch.empty_like(out)
+    tn.cgls_step(h, f0, dev(torch, y), dev(torch, w), 3, g); tn.regularize_step(h, g, 1, f1)
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), f0, 1, 3, 1, out)
+    assert torch.equal(out, f1)
+
+
+def test_twenty_outer_iterations_within_1e3(T):
+    # north_star: relative L2 <= 1e-3 after 20 outer iterations (config 1 data, K raised to 20).
+    torch, tn = T
+    cfg = workloads.config(1)
+    inp = workloads.make_inputs(cfg)
+    h, og = handles(tn, cfg)
+    y, w = inp["y"][0].astype(np.float32), inp["w"][0].astype(np.float32)
+    out = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), None, 20, cfg.m1, cfg.m2, out)
+    want = oracle.reconstruct(og, y, w, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 20, cfg.m1, cfg.m2)
+    assert rel(out.cpu().numpy(), want) < RECON_TOL
+
+
+def test_multi_slice_reconstruct_and_host_entry_points(T):
+    torch, tn = T
+    cfg = workloads.config(1, S=3, seed=4)
+    inp = workloads.make_inputs(cfg)
+    h, og = handles(tn, cfg)
+    y, w = inp["y"].astype(np.float32), inp["w"].astype(np.float32)
+    out = torch.empty(cfg.S, cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), None, 2, 3, 1, out)
+    want = oracle.reconstruct(og, y, w, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 2, 3, 1)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL * 5
+    # host-buffer entry points give the device path's result bit for bit
+    yh, wh = torch.from_numpy(y).pin_memory(), torch.from_numpy(w).pin_memory()
+    fh = torch.empty(cfg.S, cfg.N, cfg.L, cfg.L).pin_memory()
+    tn.reconstruct_host(h, yh, wh, None, 2, 3, 1, fh)
+    assert torch.equal(fh, out.cpu())
+    gh = torch.from_numpy(inp["phantom"].astype(np.float32))
+    fo = torch.empty_like(gh)
+    tn.regularize_step_host(h, gh, 2, fo)
+    od = torch.empty_like(out); tn.regularize_step(h, gh.cuda(), 2, od)
+    assert torch.equal(fo, od.cpu())
+
+
+def test_error_codes_and_launch_count(T):
+    torch, tn = T
+    cfg = workloads.config(1)
+    h, _ = handles(tn, cfg)
+    n0 = h.launch_count
+    sino = torch.empty(cfg.N, cfg.V, cfg.B, device="cuda")
+    tn.project(h, torch.zeros(cfg.N, cfg.L, cfg.L, device="cuda"), sino)
+    assert h.launch_count == n0 + 1
+    f = torch.zeros(cfg.N, cfg.L, cfg.L, device="cuda")
+    with pytest.raises(tn.TnlmError) as ei:
+        tn.cgls_step(h, f, sino, None, -1, f)
+    assert ei.value.code == 1
+    hn = tn.create(None, 16, 16, 2, 3, 3, 0.01, 0.1)
+    with pytest.raises(tn.TnlmError) as ei:
+        tn.project(hn, torch.zeros(2, 16, 16, device="cuda"), torch.zeros(2, 4, 4, device="cuda"))
+    assert ei.value.code == 1 and "geometry" in str(ei.value)
