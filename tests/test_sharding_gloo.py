@@ -1,0 +1,61 @@
+"""N>1 path on CPU: world_size-2 gloo processes exercise the slice partition, the final gather and
+the max-over-ranks timing reduction that bench.py uses.  No GPU, no oracle."""
+import os
+import socket
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_1009_1351_b200.sharding import gather_slices, max_over_ranks, slice_range
+
+
+def test_slice_range_is_a_balanced_contiguous_partition():
+    for S in [0, 1, 2, 3, 7, 64, 65]:
+        for world in [1, 2, 3, 4, 8]:
+            parts = [slice_range(S, world, r) for r in range(world)]
+            assert [i for p in parts for i in p] == list(range(S))
+            sizes = [len(p) for p in parts]
+            assert max(sizes) - min(sizes) <= 1 and sizes == sorted(sizes, reverse=True)
+    with pytest.raises(ValueError):
+        slice_range(4, 2, 2)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, S, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        mine = slice_range(S, world, rank)
+        # stand-in for per-slice results: slice s -> tensor filled with s
+        local = torch.stack([torch.full((2, 3), float(s)) for s in mine]) if len(mine) else torch.zeros(0, 2, 3)
+        full = gather_slices(local, S, dist)
+        t = max_over_ranks(10.0 + rank, dist)
+        q.put((rank, list(mine), full[:, 0, 0].tolist(), t))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("S", [5, 64])
+def test_world_size_two_gloo(S):
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, S, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res[0][1] + res[1][1] == list(range(S))
+    for _, _, gathered, t in res:
+        assert gathered == [float(s) for s in range(S)]
+        assert t == 11.0
