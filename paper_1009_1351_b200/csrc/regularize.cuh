@@ -2,215 +2,372 @@
 // cyclic neighbour phases (Eq. 3/8) inside a W x W search window
 // (L204), one Gauss-Jacobi sweep of Eq. (7) (L143-L158), optional positivity clip (L167).
 //
-// Formulation.  For one search offset delta the patch distance of every pixel is a d x d box
-// sum of ONE shifted squared-difference image SD_delta(y) = (g_i(y) - g_j(y+delta))^2.  Each
-// thread owns a 4 x 4 pixel tile and, per offset, builds the (4+2b) x (4+2b) differences from
-// registers (g_i, loaded once) and shared memory (g_j), box-sums them separably with running
-// sums (rows first, then columns), and folds the 16 distances into per-pixel softmax
-// accumulators (m, Z, A) that stay in registers for the whole window:
-//     t = -D*log2(e)/h^2 - m ;  e = 2^t ;  Z += e ;  A += e*u_j(x+delta)
-// m is a lazily updated reference exponent (raised only when some t exceeds TAU), so the
-// quotient A/Z is the softmax-weighted mean of Eq. (7) without overflow or underflow.
+// Formulation (v2, "row march").  For one search offset delta = (dr, dc) the patch distance of
+// every pixel is the d x d box sum of ONE shifted squared-difference image
+//     SD_delta(y) = (g_i(y) - g_j(y + delta))^2 ,   D(x, delta) = sum_{p in [-b,b]^2} SD_delta(x + p).
+// A warp owns a band of RB rows x 128 columns of phase i and ONE neighbour phase j ("side");
+// lane l owns the C = 4 columns 4l..4l+3.  An "item" is one dr and G = 4 consecutive dc.  For an
+// item the lane marches down the RB + 2b rows of its band: per row it loads 4+2b values of g_i
+// and 4+2b+3 values of g_j (aligned LDS.128), forms the squared differences, slides the
+// horizontal box sum over its 4 columns (2 FMA per step), adds the row into a vertical running
+// sum D[g][c] and retires the row that left the window from a 2b-deep register ring.  Every
+// D is then one FMA (exponent), one ex2.approx, one FADD (Z) and one FMA (numerator A) away from
+// the accumulators Z[row][c], A[row][c], which stay in registers for the whole window.
+// Per weight evaluation this costs 2 FSUB-slots + 2.75 FMA (box rows, x 1+2b/RB for the warm-up
+// rows) + 2 FADD (vertical) + 4: about 12 FP32 instructions against 2d+4 = 14 algorithmic flops.
+//
+// Softmax reference.  w = exp(-D/h^2)/Z is evaluated as 2^(c*(D0(x) - D(x,delta)) - 90),
+// c = log2(e)/h^2, D0 = the distance at delta = 0 (always a valid candidate), so the delta = 0
+// term is 2^-90 and Z can never underflow to 0; a candidate more than 217/c better than
+// delta = 0 overflows to +inf, which flags the pixel, and flagged pixels are recomputed by the
+// warp with the minimum-subtracted two-pass form (exact_side_ratio) straight from the shared
+// tiles.  The value is always the softmax of Eq. (3); the reference only picks the fp32 range.
+//
+// Borders.  Tiles are zero-filled outside the image (patches are zero-extended, DESIGN.md
+// reading 7).  A candidate column outside the image (or a dc beyond the window in the last
+// item of a row) gets its running sum D initialised to a huge finite value, which no sliding
+// update can change, so its weight is exactly 0 at no per-evaluation cost; candidate rows
+// outside the image are skipped warp-uniformly.
 // Weights are never stored (recomputing beats 2*W^2 floats per pixel of HBM traffic).
 #pragma once
 #include "common.cuh"
 
 namespace tnlm {
 
-constexpr int TQ = 4;           // thread tile: TQ x TQ pixels
-constexpr float TAU = 16.0f;    // lazy-rescale threshold in log2 units
+constexpr int SW_C = 4;        // columns per lane
+constexpr int SW_G = 4;        // search offsets (consecutive dc) per item
+constexpr int SW_TW = 128;     // tile width = 32 lanes x SW_C
+constexpr float SW_MARGIN = 90.0f;
 
-struct RegParams {
+struct SweepParams {
     int nx, ny, n_phase;
     int a;                  // (window-1)/2
+    int ngroups;            // ceil(window / SW_G)
+    int nb;                 // row bands per CTA; a CTA has 2*nb warps (band x side)
+    int tiles_x, tiles_y;   // tiles per image
     float neg_c;            // -log2(e)/h^2
+    float pos_c;            // +log2(e)/h^2
     float c_self;           // 1/(1+mu)
     float c_nb;             // mu/(2mu+2)
-    float big_d;            // distance given to out-of-image candidates (finite)
-    float m_init;           // initial reference exponent: neg_c*big_d/10
+    float big_d;            // distance given to excluded candidates (finite, big_d*pos_c finite)
     int clip;               // apply max(.,0) to the output
 };
 
-// Shared-memory tile layout ("planar-4"): element (row, col) of a tile lives at
-//   row*4*P + (col & 3)*P + (col >> 2),   P odd.
-// A thread reads columns 4*tx + e for several e; for a fixed e the lanes of a warp touch
-// consecutive words of one plane (and the second half-warp, four rows further down, lands 16
-// banks away because 16*P = 16 mod 32), so every LDS.32 of the inner loop is conflict-free.
-__device__ __forceinline__ int planar(int row, int col, int P) { return row * 4 * P + (col & 3) * P + (col >> 2); }
+// Shared-memory tile geometry (words), shared by host (sizing) and device.
+template <int PB>
+struct SweepGeom {
+    static constexpr int NGI = (SW_C + 2 * PB + 3) / 4;               // float4 loads of g_i per row
+    static constexpr int NGJ = (SW_C + 2 * PB + SW_G - 1 + 3) / 4;    // float4 loads of g_j per row
+    static constexpr int NUJ = (SW_C + SW_G - 1 + 3) / 4;             // float4 loads of u_j per row
+    static constexpr int GIW = 124 + 4 * NGI;                         // g_i tile row stride
+    __host__ __device__ static int gjw(int ngroups) { return 124 + 4 * (ngroups - 1) + 4 * NGJ; }
+    __host__ __device__ static int ujw(int ngroups) { return 124 + 4 * (ngroups - 1) + 4 * NUJ; }
+    __host__ __device__ static size_t smem_words(int a, int ngroups, int nb, int rb)
+    {
+        const int th = nb * rb;
+        return (size_t)(th + 2 * PB) * GIW + 2 * (size_t)(th + 2 * PB + 2 * a) * gjw(ngroups) +
+               2 * (size_t)(th + 2 * a) * ujw(ngroups) + 2 * (size_t)nb * rb * SW_TW;
+    }
+};
 
-template <int TX, int TY>
-__host__ __device__ constexpr int reg_tile_w() { return TX * TQ; }
-
-// PB = (patch-1)/2.  BORDER: the tile has candidates outside the image (or is partial).
-template <int PB, int TX, int TY, bool BORDER>
-__global__ void __launch_bounds__(TX * TY)
-gj_sweep_kernel(RegParams p, const float *__restrict__ g, const float *__restrict__ u,
-                float *__restrict__ out, const int2 *__restrict__ tiles, int tiles_per_image)
+__device__ __forceinline__ float fast_ex2(float t)
 {
-    constexpr int RW = TQ + 2 * PB;           // region side per thread
-    constexpr int TW = TX * TQ, TH = TY * TQ; // CTA pixel tile
-    const int a = p.a, halo = a + PB;
-    const int gw = TW + 2 * halo, gh = TH + 2 * halo;   // g_j tile
-    const int uw = TW + 2 * a, uh = TH + 2 * a;         // u_j tile
-    const int P = (((gw + 3) >> 2) | 1);                // odd plane stride
-    extern __shared__ float smem[];
-    float *sG = smem;                                   // gh rows
-    float *sU = smem + gh * 4 * P;                      // uh rows (same P)
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t));
+    return e;
+}
 
-    const int img = blockIdx.x / tiles_per_image;       // slice*N + phase
-    const int2 tile = tiles[blockIdx.x % tiles_per_image];
-    const int slice = img / p.n_phase, phase = img % p.n_phase;
-    const int nx = p.nx, ny = p.ny;
+// Zero-filled copy of the image window rows [r_org, r_org+rows) x cols [c_org, c_org+width)
+// into dst[rows][width]; warps take rows, lanes take columns (coalesced).
+__device__ __forceinline__ void load_tile(float *__restrict__ dst, int rows, int width,
+                                          const float *__restrict__ img, int r_org, int c_org, int ny, int nx,
+                                          int warp, int nwarps, int lane)
+{
+    for (int rr = warp; rr < rows; rr += nwarps) {
+        const int r = r_org + rr;
+        const bool rin = (unsigned)r < (unsigned)ny;
+        const float *__restrict__ src = img + (size_t)(rin ? r : 0) * nx;
+        float *__restrict__ d = dst + rr * width;
+        for (int cc = lane; cc < width; cc += 32) {
+            const int c = c_org + cc;
+            d[cc] = (rin && (unsigned)c < (unsigned)nx) ? __ldg(src + c) : 0.f;
+        }
+    }
+}
+
+// Exact (minimum-subtracted, two-pass) softmax-weighted mean of u_j over the window of ONE pixel
+// and one side, computed by the whole warp from the shared tiles: the fallback for pixels whose
+// fast-path sums overflowed.  (pr, pc) = pixel position inside the CTA tile; (r, c) = in the image.
+template <int PB>
+__device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, const float *__restrict__ sGj,
+                                               const float *__restrict__ sUj, int GJW, int UJW, int pr, int pc,
+                                               int r, int c, int a, int ny, int nx, float neg_c, int lane)
+{
+    constexpr int GIW = SweepGeom<PB>::GIW;
+    const int W = 2 * a + 1;
+    float dmin = 3.0e38f;
+    for (int pass = 0; pass < 2; ++pass) {
+        float z = 0.f, aa = 0.f, dm = 3.0e38f;
+        for (int idx = lane; idx < W * W; idx += 32) {
+            const int dr = idx / W - a, dc = idx % W - a;
+            if ((unsigned)(r + dr) >= (unsigned)ny || (unsigned)(c + dc) >= (unsigned)nx) continue;
+            float D = 0.f;
+            for (int y = 0; y <= 2 * PB; ++y)
+                for (int x = 0; x <= 2 * PB; ++x) {
+                    const float df = sGi[(pr + y) * GIW + pc + x] - sGj[(pr + dr + a + y) * GJW + pc + dc + a + x];
+                    D = fmaf(df, df, D);
+                }
+            if (pass == 0) {
+                dm = fminf(dm, D);
+            } else {
+                const float e = exp2f(neg_c * (D - dmin));
+                z += e;
+                aa = fmaf(e, sUj[(pr + dr + a) * UJW + pc + dc + a], aa);
+            }
+        }
+        if (pass == 0) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) dm = fminf(dm, __shfl_xor_sync(0xffffffffu, dm, o));
+            dmin = dm;
+        } else {
+            z = warp_sum(z);
+            aa = warp_sum(aa);
+            return aa / z;
+        }
+    }
+    return 0.f;
+}
+
+// One Gauss-Jacobi sweep of Eq. (7) for every pixel of every phase of every slice.
+// grid.x = (S*N) * tiles_y * tiles_x; block = 64 * nb threads; warp w: band = w >> 1, side = w & 1.
+template <int PB, int RB>
+__global__ void __launch_bounds__(256, 1)
+gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out)
+{
+    using GEO = SweepGeom<PB>;
+    constexpr int C = SW_C, G = SW_G, NGI = GEO::NGI, NGJ = GEO::NGJ, NUJ = GEO::NUJ, GIW = GEO::GIW;
+    constexpr int NQ = C + 2 * PB;             // squared differences per offset and row
+    constexpr int RING = (PB > 0) ? 2 * PB : 1;
+    const int a = p.a, ng = p.ngroups, nb = p.nb, nx = p.nx, ny = p.ny;
+    const int TH = nb * RB;
+    const int GJW = GEO::gjw(ng), UJW = GEO::ujw(ng);
+    const int gi_rows = TH + 2 * PB, gj_rows = TH + 2 * PB + 2 * a, uj_rows = TH + 2 * a;
+
+    extern __shared__ float4 smem4[];
+    float *sGi = reinterpret_cast<float *>(smem4);
+    float *sGj = sGi + gi_rows * GIW;              // [2][gj_rows][GJW]
+    float *sUj = sGj + 2 * gj_rows * GJW;          // [2][uj_rows][UJW]
+    float *sK = sUj + 2 * uj_rows * UJW;           // [2*nb][RB][128]
+
+    const int tiles_per_img = p.tiles_x * p.tiles_y;
+    const int img = blockIdx.x / tiles_per_img;    // slice*N + phase
+    const int tl = blockIdx.x - img * tiles_per_img;
+    const int tile_r0 = (tl / p.tiles_x) * TH, tile_c0 = (tl % p.tiles_x) * SW_TW;
+    const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
     const size_t npix = (size_t)nx * ny;
-    const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
-    const int r0 = tile.y + ty * TQ, c0 = tile.x + tx * TQ;    // thread's first pixel
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = 2 * nb;
 
-    // g_i region of this thread: (r0-PB .. r0+TQ-1+PB) x (c0-PB .. c0+TQ-1+PB), zero outside.
-    const float *__restrict__ gi = g + ((size_t)slice * p.n_phase + phase) * npix;
-    float Gi[RW][RW];
+    {   // stage g_i, and g_j / u_j of both cyclic neighbours (L81), zero-filled outside the image
+        const float *__restrict__ gi = g + (size_t)img * npix;
+        load_tile(sGi, gi_rows, GIW, gi, tile_r0 - PB, tile_c0 - PB, ny, nx, warp, nwarps, lane);
 #pragma unroll
-    for (int rr = 0; rr < RW; ++rr)
-#pragma unroll
-        for (int cc = 0; cc < RW; ++cc) {
-            const int r = r0 - PB + rr, c = c0 - PB + cc;
-            Gi[rr][cc] = ((unsigned)r < (unsigned)ny && (unsigned)c < (unsigned)nx) ? __ldg(gi + (size_t)r * nx + c) : 0.f;
+        for (int s = 0; s < 2; ++s) {
+            const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
+            const size_t jo = ((size_t)slice * p.n_phase + j) * npix;
+            load_tile(sGj + s * gj_rows * GJW, gj_rows, GJW, g + jo, tile_r0 - PB - a, tile_c0 - PB - a, ny, nx,
+                      warp, nwarps, lane);
+            load_tile(sUj + s * uj_rows * UJW, uj_rows, UJW, u + jo, tile_r0 - a, tile_c0 - a, ny, nx, warp,
+                      nwarps, lane);
         }
+    }
+    __syncthreads();
 
-    float nbsum[TQ][TQ];
-#pragma unroll
-    for (int rr = 0; rr < TQ; ++rr)
-#pragma unroll
-        for (int q = 0; q < TQ; ++q) nbsum[rr][q] = 0.f;
+    const int side = warp & 1, band = warp >> 1;
+    const int lr0 = band * RB;                     // first pixel row of the band inside the tile
+    const int r0 = tile_r0 + lr0, c0 = tile_c0 + C * lane;
+    const float *__restrict__ myGj = sGj + side * gj_rows * GJW;
+    const float *__restrict__ myUj = sUj + side * uj_rows * UJW;
+    float *__restrict__ myK = sK + warp * RB * SW_TW;
 
-    // per-thread smem base offsets (tile row 4*ty, column 4*tx => plane 0, index tx)
-    const int rowstride = 4 * P;
-    const int tbase = (ty * TQ) * rowstride + tx;
-
-    for (int side = 0; side < 2; ++side) {
-        const int j = (phase + (side == 0 ? p.n_phase - 1 : 1)) % p.n_phase;   // cyclic (L81)
-        const float *__restrict__ gj = g + ((size_t)slice * p.n_phase + j) * npix;
-        const float *__restrict__ uj = u + ((size_t)slice * p.n_phase + j) * npix;
-        __syncthreads();                                   // previous side's readers are done
-        for (int idx = threadIdx.x; idx < gh * gw; idx += TX * TY) {
-            const int rr = idx / gw, cc = idx - rr * gw;
-            const int r = tile.y - halo + rr, c = tile.x - halo + cc;
-            sG[planar(rr, cc, P)] = ((unsigned)r < (unsigned)ny && (unsigned)c < (unsigned)nx) ? __ldg(gj + (size_t)r * nx + c) : 0.f;
-        }
-        for (int idx = threadIdx.x; idx < uh * uw; idx += TX * TY) {
-            const int rr = idx / uw, cc = idx - rr * uw;
-            const int r = tile.y - a + rr, c = tile.x - a + cc;
-            sU[planar(rr, cc, P)] = ((unsigned)r < (unsigned)ny && (unsigned)c < (unsigned)nx) ? __ldg(uj + (size_t)r * nx + c) : 0.f;
-        }
-        __syncthreads();
-
-        float m[TQ][TQ], Z[TQ][TQ], A[TQ][TQ];
+    // ---- reference exponents K(x) = c*D0(x) - 90, D0 = distance at delta = 0 (same march, one offset)
+    {
+        float D0[C], ring[C][RING];
 #pragma unroll
-        for (int rr = 0; rr < TQ; ++rr)
+        for (int c = 0; c < C; ++c) D0[c] = 0.f;
+        const float *__restrict__ gip = sGi + lr0 * GIW + C * lane;
+        const float *__restrict__ gjp = myGj + (lr0 + a) * GJW + C * lane + a;
 #pragma unroll
-            for (int q = 0; q < TQ; ++q) { m[rr][q] = p.m_init; Z[rr][q] = 0.f; A[rr][q] = 0.f; }
-
-        for (int dr = -a; dr <= a; ++dr) {
-            float rowpen[TQ];
-            if (BORDER) {
+        for (int s = 0; s < RB + 2 * PB; ++s) {
+            float sd[NQ], H[C];
 #pragma unroll
-                for (int rr = 0; rr < TQ; ++rr) rowpen[rr] = ((unsigned)(r0 + rr + dr) < (unsigned)ny) ? 0.f : p.big_d;
+            for (int q = 0; q < NQ; ++q) sd[q] = gip[s * GIW + q] - gjp[s * GJW + q];
+            float h = sd[0] * sd[0];
+#pragma unroll
+            for (int q = 1; q <= 2 * PB; ++q) h = fmaf(sd[q], sd[q], h);
+            H[0] = h;
+#pragma unroll
+            for (int c = 1; c < C; ++c) {
+                h = fmaf(sd[c + 2 * PB], sd[c + 2 * PB], h);
+                h = fmaf(-sd[c - 1], sd[c - 1], h);
+                H[c] = h;
             }
-            const int gbase = tbase + (dr + a) * rowstride;   // g_j tile row (4ty + rr' + dr + a)
-            for (int dc = -a; dc <= a; ++dc) {
-                // column offsets inside a tile row for e = j + dc + a, j = 0..RW-1
-                int off[RW];
 #pragma unroll
-                for (int jj = 0; jj < RW; ++jj) {
-                    const int e = jj + dc + a;
-                    off[jj] = (e & 3) * P + (e >> 2);
+            for (int c = 0; c < C; ++c) {
+                D0[c] += H[c];
+                if (s >= 2 * PB) {
+                    myK[(s - 2 * PB) * SW_TW + C * lane + c] = fmaf(D0[c], p.pos_c, -SW_MARGIN);
+                    D0[c] -= (PB > 0) ? ring[c][s % RING] : H[c];
                 }
-                // ---- rows of the region: differences, horizontal running box sums
-                float H[RW][TQ];
-#pragma unroll
-                for (int rr = 0; rr < RW; ++rr) {
-                    float df[RW];
-#pragma unroll
-                    for (int jj = 0; jj < RW; ++jj) df[jj] = Gi[rr][jj] - sG[gbase + rr * rowstride + off[jj]];
-                    float h0 = df[0] * df[0];
-#pragma unroll
-                    for (int jj = 1; jj <= 2 * PB; ++jj) h0 = fmaf(df[jj], df[jj], h0);
-                    H[rr][0] = h0;
-#pragma unroll
-                    for (int q = 1; q < TQ; ++q) {
-                        h0 = fmaf(df[q + 2 * PB], df[q + 2 * PB], h0);
-                        h0 = fmaf(-df[q - 1], df[q - 1], h0);
-                        H[rr][q] = h0;
-                    }
-                }
-                // ---- vertical running box sums -> D, then exponent relative to m
-                float t[TQ][TQ], Dd[TQ][TQ];
-#pragma unroll
-                for (int q = 0; q < TQ; ++q) {
-                    float colpen = 0.f;
-                    if (BORDER) colpen = ((unsigned)(c0 + q + dc) < (unsigned)nx) ? 0.f : p.big_d;
-                    float d0 = H[0][q];
-#pragma unroll
-                    for (int rr = 1; rr <= 2 * PB; ++rr) d0 += H[rr][q];
-#pragma unroll
-                    for (int rr = 0; rr < TQ; ++rr) {
-                        if (rr > 0) d0 = (d0 + H[rr + 2 * PB][q]) - H[rr - 1][q];
-                        float dv = d0;
-                        if (BORDER) dv = fmaxf(fmaxf(dv, rowpen[rr]), colpen);
-                        Dd[rr][q] = dv;
-                        t[rr][q] = fmaf(dv, p.neg_c, -m[rr][q]);
-                    }
-                }
-                // ---- lazy rescale: rare once the window's best matches have been seen
-                float tmax = t[0][0];
-#pragma unroll
-                for (int rr = 0; rr < TQ; ++rr)
-#pragma unroll
-                    for (int q = 0; q < TQ; ++q) tmax = fmaxf(tmax, t[rr][q]);
-                if (tmax > TAU) {
-#pragma unroll
-                    for (int rr = 0; rr < TQ; ++rr)
-#pragma unroll
-                        for (int q = 0; q < TQ; ++q)
-                            if (t[rr][q] > TAU) {
-                                const float s = Dd[rr][q] * p.neg_c;
-                                const float corr = exp2f(m[rr][q] - s);
-                                Z[rr][q] *= corr;
-                                A[rr][q] *= corr;
-                                m[rr][q] = s;
-                                t[rr][q] = 0.f;
-                            }
-                }
-                // ---- accumulate
-                const int ubase = tbase + (dr + a) * rowstride;   // u_j tile row (4ty + rr + dr + a)
-#pragma unroll
-                for (int rr = 0; rr < TQ; ++rr)
-#pragma unroll
-                    for (int q = 0; q < TQ; ++q) {
-                        float e;
-                        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t[rr][q]));
-                        Z[rr][q] += e;
-                        A[rr][q] = fmaf(e, sU[ubase + rr * rowstride + off[q]], A[rr][q]);
-                    }
+                ring[c][s % RING] = H[c];
             }
         }
+    }
+    __syncwarp();
+
+    // ---- the window: items (dr, 4 consecutive dc), accumulators in registers
+    float Z[RB][C], A[RB][C];
 #pragma unroll
-        for (int rr = 0; rr < TQ; ++rr)
+    for (int rr = 0; rr < RB; ++rr)
 #pragma unroll
-            for (int q = 0; q < TQ; ++q) nbsum[rr][q] += __fdividef(A[rr][q], Z[rr][q]);
+        for (int c = 0; c < C; ++c) { Z[rr][c] = 0.f; A[rr][c] = 0.f; }
+
+    for (int dr = -a; dr <= a; ++dr) {
+        unsigned okmask = 0;                       // pixel row and candidate row inside the image
+#pragma unroll
+        for (int rr = 0; rr < RB; ++rr)
+            if (r0 + rr < ny && (unsigned)(r0 + rr + dr) < (unsigned)ny) okmask |= 1u << rr;
+        if (okmask == 0) continue;
+        for (int dcg = 0; dcg < ng; ++dcg) {
+            const int dc0 = -a + G * dcg;
+            float D[G][C], ring[G][C][RING];
+#pragma unroll
+            for (int gg = 0; gg < G; ++gg)
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    const int col = c0 + c + dc0 + gg;
+                    D[gg][c] = (dc0 + gg <= a && (unsigned)col < (unsigned)nx) ? 0.f : p.big_d;
+                }
+            const float4 *__restrict__ gip = reinterpret_cast<const float4 *>(sGi + lr0 * GIW) + lane;
+            const float4 *__restrict__ gjp = reinterpret_cast<const float4 *>(myGj + (lr0 + dr + a) * GJW) + lane + dcg;
+            const float4 *__restrict__ ujp = reinterpret_cast<const float4 *>(myUj + (lr0 + dr + a) * UJW) + lane + dcg;
+            const float4 *__restrict__ kp = reinterpret_cast<const float4 *>(myK) + lane;
+#pragma unroll
+            for (int s = 0; s < RB + 2 * PB; ++s) {
+                float gi_[4 * NGI], gj_[4 * NGJ];
+#pragma unroll
+                for (int k = 0; k < NGI; ++k) {
+                    const float4 v = gip[s * (GIW / 4) + k];
+                    gi_[4 * k] = v.x; gi_[4 * k + 1] = v.y; gi_[4 * k + 2] = v.z; gi_[4 * k + 3] = v.w;
+                }
+#pragma unroll
+                for (int k = 0; k < NGJ; ++k) {
+                    const float4 v = gjp[s * (GJW / 4) + k];
+                    gj_[4 * k] = v.x; gj_[4 * k + 1] = v.y; gj_[4 * k + 2] = v.z; gj_[4 * k + 3] = v.w;
+                }
+                // squared differences and horizontal box sums of this row, all G offsets
+                float H[G][C];
+#pragma unroll
+                for (int gg = 0; gg < G; ++gg) {
+                    float sd[NQ];
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) sd[q] = gi_[q] - gj_[q + gg];
+                    float h = sd[0] * sd[0];
+#pragma unroll
+                    for (int q = 1; q <= 2 * PB; ++q) h = fmaf(sd[q], sd[q], h);
+                    H[gg][0] = h;
+#pragma unroll
+                    for (int c = 1; c < C; ++c) {
+                        h = fmaf(sd[c + 2 * PB], sd[c + 2 * PB], h);
+                        h = fmaf(-sd[c - 1], sd[c - 1], h);
+                        H[gg][c] = h;
+                    }
+                }
+#pragma unroll
+                for (int gg = 0; gg < G; ++gg)
+#pragma unroll
+                    for (int c = 0; c < C; ++c) D[gg][c] += H[gg][c];
+                if (s >= 2 * PB) {                 // the window of pixel row rr is complete
+                    const int rr = s - 2 * PB;
+                    // rows whose pixel or candidate row is outside the image get K = -huge: weight 0
+                    const bool ok = (okmask >> rr) & 1u;
+                    float uj_[4 * NUJ], K_[C];
+#pragma unroll
+                    for (int k = 0; k < NUJ; ++k) {
+                        const float4 v = ujp[rr * (UJW / 4) + k];
+                        uj_[4 * k] = v.x; uj_[4 * k + 1] = v.y; uj_[4 * k + 2] = v.z; uj_[4 * k + 3] = v.w;
+                    }
+                    const float4 kv = kp[rr * (SW_TW / 4)];
+                    K_[0] = ok ? kv.x : -1.0e30f; K_[1] = ok ? kv.y : -1.0e30f;
+                    K_[2] = ok ? kv.z : -1.0e30f; K_[3] = ok ? kv.w : -1.0e30f;
+#pragma unroll
+                    for (int gg = 0; gg < G; ++gg)
+#pragma unroll
+                        for (int c = 0; c < C; ++c) {
+                            const float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
+                            Z[rr][c] += e;
+                            A[rr][c] = fmaf(e, uj_[c + gg], A[rr][c]);
+                            D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[gg][c];
+                        }
+                }
+#pragma unroll
+                for (int gg = 0; gg < G; ++gg)
+#pragma unroll
+                    for (int c = 0; c < C; ++c) ring[gg][c][s % RING] = H[gg][c];
+            }
+        }
     }
 
-    float *__restrict__ o = out + ((size_t)slice * p.n_phase + phase) * npix;
+    // ---- softmax-weighted mean per pixel; overflowed pixels take the exact two-pass route
 #pragma unroll
-    for (int rr = 0; rr < TQ; ++rr)
+    for (int rr = 0; rr < RB; ++rr)
 #pragma unroll
-        for (int q = 0; q < TQ; ++q) {
-            const int r = r0 + rr, c = c0 + q;
-            if (r < ny && c < nx) {
-                float v = fmaf(p.c_nb, nbsum[rr][q], p.c_self * Gi[rr + PB][q + PB]);
-                if (p.clip) v = fmaxf(v, 0.f);
-                o[(size_t)r * nx + c] = v;
+        for (int c = 0; c < C; ++c) {
+            const bool valid = (r0 + rr < ny) && (c0 + c < nx);
+            const bool bad = valid && !(Z[rr][c] < 1.0e38f);
+            A[rr][c] = A[rr][c] / Z[rr][c];
+            unsigned m = __ballot_sync(0xffffffffu, bad);
+            while (m) {
+                const int L = __ffs(m) - 1;
+                m &= m - 1;
+                const float v = exact_side_ratio<PB>(sGi, myGj, myUj, GJW, UJW, lr0 + rr, C * L + c, r0 + rr,
+                                                     tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane);
+                if (lane == L) A[rr][c] = v;
             }
         }
+
+    // ---- combine the two sides (Eq. 7): side-1 warps hand their means to the side-0 warp of the band
+    if (side == 1) {
+#pragma unroll
+        for (int rr = 0; rr < RB; ++rr)
+            reinterpret_cast<float4 *>(myK)[rr * (SW_TW / 4) + lane] = make_float4(A[rr][0], A[rr][1], A[rr][2], A[rr][3]);
+    }
+    __syncthreads();
+    if (side == 0) {
+        const float *__restrict__ other = sK + (warp + 1) * RB * SW_TW;
+        float *__restrict__ o = out + (size_t)img * npix;
+        const bool vec = ((nx & 3) == 0) && ((reinterpret_cast<uintptr_t>(out) & 15) == 0) && (c0 + C <= nx);
+#pragma unroll
+        for (int rr = 0; rr < RB; ++rr) {
+            const int r = r0 + rr;
+            if (r >= ny) break;
+            const float4 ov = reinterpret_cast<const float4 *>(other)[rr * (SW_TW / 4) + lane];
+            const float on[C] = {ov.x, ov.y, ov.z, ov.w};
+            float v[C];
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                const float gc = sGi[(lr0 + rr + PB) * GIW + C * lane + PB + c];
+                v[c] = fmaf(p.c_nb, A[rr][c] + on[c], p.c_self * gc);
+                if (p.clip) v[c] = fmaxf(v[c], 0.f);
+            }
+            if (vec) {
+                *reinterpret_cast<float4 *>(o + (size_t)r * nx + c0) = make_float4(v[0], v[1], v[2], v[3]);
+            } else {
+#pragma unroll
+                for (int c = 0; c < C; ++c)
+                    if (c0 + c < nx) o[(size_t)r * nx + c0 + c] = v[c];
+            }
+        }
+    }
 }
 
 // f = max(g, 0): the m2 = 0 case of steps 3-5.

@@ -1,6 +1,7 @@
 // tnlm_api.cu -- C ABI of libtnlm (see include/tnlm.h): handle, argument checks, workspace,
 // and the launch sequences of the five operations.  Host code only orchestrates; every step
 // of the path runs in the kernels of projector.cuh, cgls.cuh and regularize.cuh.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -17,22 +18,26 @@
 using namespace tnlm;
 
 static constexpr int MAX_PATCH = 9, MAX_WINDOW = 31;
-static constexpr int REG_TX = 16, REG_TY = 8;          // CTA = 128 threads, 64 x 32 pixel tile
+
+// One compiled shape of gj_sweep_kernel<PB, RB> with nb row bands per CTA (regularize.cuh).
+struct SweepShape {
+    const void *fn = nullptr;
+    int rb = 0, nb = 0, occ = 0;    // rows per band, bands per CTA, resident CTAs per SM
+    size_t smem = 0;
+};
 
 struct tnlm_handle {
     int nx = 0, ny = 0, n_phase = 0, window = 0, patch = 0;
     float h = 0.f, mu = 0.f;
     bool has_geom = false;
     Geom G{};
-    RegParams R{};
+    SweepParams R{};
+    std::vector<SweepShape> shapes;   // launchable sweep shapes for this (window, patch)
+    int n_sm = 148;
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
     float4 *d_views = nullptr;
-    // TNLM tile lists (device): interior tiles first, then border tiles
-    int2 *d_tiles = nullptr;
-    int n_interior = 0, n_border = 0;
-    size_t reg_smem = 0;
     // workspace, sized for ws_slices
     int ws_slices = 0;
     float *d_s = nullptr, *d_t = nullptr, *d_g = nullptr, *d_f = nullptr;  // images
@@ -120,20 +125,60 @@ static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, st
         }
 }
 
-static size_t reg_smem_bytes(int window, int patch)
+// Every compiled (PB, RB) of gj_sweep_kernel, with nb in {4, 2, 1}, that fits one CTA's shared
+// memory becomes a SweepShape; the launcher picks the cheapest one for the image count at hand.
+template <int PB, int RB>
+static cudaError_t add_sweep_shapes(tnlm_handle *H, size_t smem_limit)
 {
-    const int a = (window - 1) / 2, b = (patch - 1) / 2, halo = a + b;
-    const int TW = REG_TX * TQ, TH = REG_TY * TQ;
-    const int gw = TW + 2 * halo, gh = TH + 2 * halo, uh = TH + 2 * a;
-    const int P = (((gw + 3) >> 2) | 1);
-    return (size_t)(gh + uh) * 4 * P * sizeof(float);
+    const void *fn = (const void *)gj_sweep_kernel<PB, RB>;
+    size_t biggest = 0;
+    std::vector<SweepShape> mine;
+    for (int nb = 4; nb >= 1; nb >>= 1) {
+        SweepShape sh;
+        sh.fn = fn; sh.rb = RB; sh.nb = nb;
+        sh.smem = SweepGeom<PB>::smem_words(H->R.a, H->R.ngroups, nb, RB) * sizeof(float);
+        if (sh.smem > smem_limit) continue;
+        if (sh.smem > biggest) biggest = sh.smem;
+        mine.push_back(sh);
+    }
+    if (mine.empty()) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)biggest);
+    if (e != cudaSuccess) return e;
+    for (SweepShape &sh : mine) {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&sh.occ, fn, 64 * sh.nb, sh.smem);
+        if (e != cudaSuccess) return e;
+        if (sh.occ >= 1) H->shapes.push_back(sh);
+    }
+    return cudaSuccess;
 }
 
-template <int PB, bool BORDER>
-static cudaError_t set_reg_attr(size_t smem)
+static cudaError_t build_sweep_shapes(tnlm_handle *H, size_t smem_limit)
 {
-    return cudaFuncSetAttribute(gj_sweep_kernel<PB, REG_TX, REG_TY, BORDER>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaSuccess;
+    switch ((H->patch - 1) / 2) {
+        case 0: e = add_sweep_shapes<0, 8>(H, smem_limit); if (e == cudaSuccess) e = add_sweep_shapes<0, 10>(H, smem_limit); break;
+        case 1: e = add_sweep_shapes<1, 8>(H, smem_limit); if (e == cudaSuccess) e = add_sweep_shapes<1, 10>(H, smem_limit); break;
+        case 2: e = add_sweep_shapes<2, 8>(H, smem_limit); if (e == cudaSuccess) e = add_sweep_shapes<2, 10>(H, smem_limit); break;
+        case 3: e = add_sweep_shapes<3, 8>(H, smem_limit); break;
+        default: e = add_sweep_shapes<4, 4>(H, smem_limit); break;
+    }
+    return e;
+}
+
+// Cost model of one sweep over n_img images with shape sh, in (resident warps) x (rows marched)
+// per SM: full waves of occ CTAs per SM, then the remainder spread over the SMs.  At least 8
+// warps per SM are needed to keep the FP32 pipes busy, so fewer do not run faster.
+static double sweep_cost(const tnlm_handle *H, const SweepShape &sh, int n_img)
+{
+    const int pb = (H->patch - 1) / 2;
+    const long long th = (long long)sh.nb * sh.rb;
+    const long long ctas = (long long)n_img * ((H->ny + th - 1) / th) * ((H->nx + SW_TW - 1) / SW_TW);
+    const long long cap = (long long)H->n_sm * sh.occ;
+    const long long full = ctas / cap, rem = ctas % cap;
+    auto wave = [&](long long k) { return (double)std::max<long long>(k * 2 * sh.nb, 8) * (sh.rb + 2 * pb); };
+    double c = (double)full * wave(sh.occ);
+    if (rem) c += wave((rem + H->n_sm - 1) / H->n_sm);
+    return c;
 }
 
 extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_phase, int window, int patch,
@@ -171,45 +216,22 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     H->nx = nx; H->ny = ny; H->n_phase = n_phase; H->window = window; H->patch = patch; H->h = h; H->mu = mu;
 
     // TNLM parameters
-    RegParams &R = H->R;
+    SweepParams &R = H->R;
     R.nx = nx; R.ny = ny; R.n_phase = n_phase; R.a = (window - 1) / 2;
+    R.ngroups = (window + SW_G - 1) / SW_G;
     const double c = 1.4426950408889634 / ((double)h * (double)h);
     R.neg_c = (float)(-c);
+    R.pos_c = (float)c;
     R.c_self = (float)(1.0 / (1.0 + (double)mu));
     R.c_nb = (float)((double)mu / (2.0 * (double)mu + 2.0));
-    R.big_d = (float)std::fmin(1e37, 1e30 / c);
-    R.m_init = R.neg_c * R.big_d * 0.1f;
+    R.big_d = (float)std::fmin(1e30, 1e37 / c);
     R.clip = 0;
-    H->reg_smem = reg_smem_bytes(window, patch);
-    if (H->reg_smem > (size_t)prop.sharedMemPerBlockOptin) {
+    H->n_sm = prop.multiProcessorCount;
+    ce = build_sweep_shapes(H, (size_t)prop.sharedMemPerBlockOptin);
+    if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "sweep kernel setup"); }
+    if (H->shapes.empty()) {
         delete H;
         return fail(nullptr, TNLM_UNSUPPORTED, "window/patch need more shared memory than one CTA has");
-    }
-    {
-        cudaError_t e = cudaSuccess;
-        switch ((patch - 1) / 2) {
-            case 0: e = set_reg_attr<0, false>(H->reg_smem); if (e == cudaSuccess) e = set_reg_attr<0, true>(H->reg_smem); break;
-            case 1: e = set_reg_attr<1, false>(H->reg_smem); if (e == cudaSuccess) e = set_reg_attr<1, true>(H->reg_smem); break;
-            case 2: e = set_reg_attr<2, false>(H->reg_smem); if (e == cudaSuccess) e = set_reg_attr<2, true>(H->reg_smem); break;
-            case 3: e = set_reg_attr<3, false>(H->reg_smem); if (e == cudaSuccess) e = set_reg_attr<3, true>(H->reg_smem); break;
-            default: e = set_reg_attr<4, false>(H->reg_smem); if (e == cudaSuccess) e = set_reg_attr<4, true>(H->reg_smem); break;
-        }
-        if (e != cudaSuccess) { delete H; return cuda_fail(nullptr, e, "cudaFuncSetAttribute"); }
-    }
-    // tile lists
-    {
-        const int TW = REG_TX * TQ, TH = REG_TY * TQ, a = R.a;
-        std::vector<int2> inner, border;
-        for (int ty = 0; ty < ny; ty += TH)
-            for (int tx = 0; tx < nx; tx += TW) {
-                const bool in = tx - a >= 0 && ty - a >= 0 && tx + TW - 1 + a <= nx - 1 && ty + TH - 1 + a <= ny - 1;
-                (in ? inner : border).push_back(make_int2(tx, ty));
-            }
-        H->n_interior = (int)inner.size(); H->n_border = (int)border.size();
-        inner.insert(inner.end(), border.begin(), border.end());
-        if (cudaMalloc(&H->d_tiles, inner.size() * sizeof(int2)) != cudaSuccess) { delete H; return fail(nullptr, TNLM_ALLOC_FAILED, "device allocation failed (tiles)"); }
-        ce = cudaMemcpy(H->d_tiles, inner.data(), inner.size() * sizeof(int2), cudaMemcpyHostToDevice);
-        if (ce != cudaSuccess) { cudaFree(H->d_tiles); delete H; return cuda_fail(nullptr, ce, "cudaMemcpy tiles"); }
     }
     if (geometry) {
         const tnlm_geometry &g = *geometry;
@@ -253,7 +275,6 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     if (H->d_tab) cudaFree(H->d_tab);
     if (H->d_rng) cudaFree(H->d_rng);
     if (H->d_views) cudaFree(H->d_views);
-    if (H->d_tiles) cudaFree(H->d_tiles);
     delete H;
     return TNLM_OK;
 }
@@ -377,35 +398,28 @@ extern "C" int tnlm_cgls_step(tnlm_handle *H, const float *f_in, const float *y,
 }
 
 // ------------------------------------------------------------------------------ TNLM
-template <int PB>
-static int launch_sweep_pb(tnlm_handle *H, const float *g, const float *u, float *out, int clip, int n_slices, cudaStream_t st)
-{
-    RegParams R = H->R;
-    R.clip = clip;
-    const int nimg = n_slices * H->n_phase;
-    const int per = H->n_interior + H->n_border;
-    if (H->n_interior > 0) {
-        gj_sweep_kernel<PB, REG_TX, REG_TY, false><<<H->n_interior * nimg, REG_TX * REG_TY, H->reg_smem, st>>>(
-            R, g, u, out, H->d_tiles, H->n_interior);
-        LAUNCHED(H);
-    }
-    if (H->n_border > 0) {
-        gj_sweep_kernel<PB, REG_TX, REG_TY, true><<<H->n_border * nimg, REG_TX * REG_TY, H->reg_smem, st>>>(
-            R, g, u, out, H->d_tiles + H->n_interior, H->n_border);
-        LAUNCHED(H);
-    }
-    (void)per;
-    return TNLM_OK;
-}
 static int launch_sweep(tnlm_handle *H, const float *g, const float *u, float *out, int clip, int n_slices, cudaStream_t st)
 {
-    switch ((H->patch - 1) / 2) {
-        case 0: return launch_sweep_pb<0>(H, g, u, out, clip, n_slices, st);
-        case 1: return launch_sweep_pb<1>(H, g, u, out, clip, n_slices, st);
-        case 2: return launch_sweep_pb<2>(H, g, u, out, clip, n_slices, st);
-        case 3: return launch_sweep_pb<3>(H, g, u, out, clip, n_slices, st);
-        default: return launch_sweep_pb<4>(H, g, u, out, clip, n_slices, st);
+    const int nimg = n_slices * H->n_phase;
+    const SweepShape *best = nullptr;
+    double best_cost = 0.0;
+    for (const SweepShape &sh : H->shapes) {
+        const double c = sweep_cost(H, sh, nimg);
+        if (!best || c < best_cost) { best = &sh; best_cost = c; }
     }
+    SweepParams R = H->R;
+    R.clip = clip;
+    R.nb = best->nb;
+    const int th = best->nb * best->rb;
+    R.tiles_x = (H->nx + SW_TW - 1) / SW_TW;
+    R.tiles_y = (H->ny + th - 1) / th;
+    const long long ctas = (long long)nimg * R.tiles_x * R.tiles_y;
+    if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
+    void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out};
+    cudaError_t e = cudaLaunchKernel(best->fn, dim3((unsigned)ctas), dim3(64 * best->nb), args, best->smem, st);
+    if (e != cudaSuccess) return cuda_fail(H, e, "cudaLaunchKernel(gj_sweep_kernel)");
+    LAUNCHED(H);
+    return TNLM_OK;
 }
 
 // g -> f_out; g and f_out are distinct device buffers or the same buffer.
