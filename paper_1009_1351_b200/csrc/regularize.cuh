@@ -38,6 +38,12 @@ constexpr int SW_C = 4;        // columns per lane
 constexpr int SW_G = 4;        // search offsets (consecutive dc) per item
 constexpr int SW_TW = 128;     // tile width = 32 lanes x SW_C
 constexpr float SW_MARGIN = 90.0f;
+// Keeps ptxas from hoisting the next row's shared-memory loads over a whole march step (the
+// hoisted values push the kernel over 255 registers and spill); the other warp of the scheduler
+// covers the exposed load latency.
+#ifndef SW_STEP_FENCE
+#define SW_STEP_FENCE() asm volatile("" ::: "memory")
+#endif
 
 struct SweepParams {
     int nx, ny, n_phase;
@@ -264,33 +270,11 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                     const float4 v = gjp[s * (GJW / 4) + k];
                     gj_[4 * k] = v.x; gj_[4 * k + 1] = v.y; gj_[4 * k + 2] = v.z; gj_[4 * k + 3] = v.w;
                 }
-                // squared differences and horizontal box sums of this row, all G offsets
-                float H[G][C];
-#pragma unroll
-                for (int gg = 0; gg < G; ++gg) {
-                    float sd[NQ];
-#pragma unroll
-                    for (int q = 0; q < NQ; ++q) sd[q] = gi_[q] - gj_[q + gg];
-                    float h = sd[0] * sd[0];
-#pragma unroll
-                    for (int q = 1; q <= 2 * PB; ++q) h = fmaf(sd[q], sd[q], h);
-                    H[gg][0] = h;
-#pragma unroll
-                    for (int c = 1; c < C; ++c) {
-                        h = fmaf(sd[c + 2 * PB], sd[c + 2 * PB], h);
-                        h = fmaf(-sd[c - 1], sd[c - 1], h);
-                        H[gg][c] = h;
-                    }
-                }
-#pragma unroll
-                for (int gg = 0; gg < G; ++gg)
-#pragma unroll
-                    for (int c = 0; c < C; ++c) D[gg][c] += H[gg][c];
-                if (s >= 2 * PB) {                 // the window of pixel row rr is complete
+                float uj_[4 * NUJ], K_[C];
+                if (s >= 2 * PB) {                 // this step completes the window of pixel row rr
                     const int rr = s - 2 * PB;
                     // rows whose pixel or candidate row is outside the image get K = -huge: weight 0
                     const bool ok = (okmask >> rr) & 1u;
-                    float uj_[4 * NUJ], K_[C];
 #pragma unroll
                     for (int k = 0; k < NUJ; ++k) {
                         const float4 v = ujp[rr * (UJW / 4) + k];
@@ -299,20 +283,37 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                     const float4 kv = kp[rr * (SW_TW / 4)];
                     K_[0] = ok ? kv.x : -1.0e30f; K_[1] = ok ? kv.y : -1.0e30f;
                     K_[2] = ok ? kv.z : -1.0e30f; K_[3] = ok ? kv.w : -1.0e30f;
+                }
 #pragma unroll
-                    for (int gg = 0; gg < G; ++gg)
+                for (int gg = 0; gg < G; ++gg) {
+                    // squared differences and the horizontal box sums of this row for offset gg
+                    float sd[NQ], H[C];
 #pragma unroll
-                        for (int c = 0; c < C; ++c) {
+                    for (int q = 0; q < NQ; ++q) sd[q] = gi_[q] - gj_[q + gg];
+                    float h = sd[0] * sd[0];
+#pragma unroll
+                    for (int q = 1; q <= 2 * PB; ++q) h = fmaf(sd[q], sd[q], h);
+                    H[0] = h;
+#pragma unroll
+                    for (int c = 1; c < C; ++c) {
+                        h = fmaf(sd[c + 2 * PB], sd[c + 2 * PB], h);
+                        h = fmaf(-sd[c - 1], sd[c - 1], h);
+                        H[c] = h;
+                    }
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        D[gg][c] += H[c];
+                        if (s >= 2 * PB) {
+                            const int rr = s - 2 * PB;
                             const float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
                             Z[rr][c] += e;
                             A[rr][c] = fmaf(e, uj_[c + gg], A[rr][c]);
-                            D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[gg][c];
+                            D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[c];
                         }
+                        ring[gg][c][s % RING] = H[c];
+                    }
                 }
-#pragma unroll
-                for (int gg = 0; gg < G; ++gg)
-#pragma unroll
-                    for (int c = 0; c < C; ++c) ring[gg][c][s % RING] = H[gg][c];
+                SW_STEP_FENCE();
             }
         }
     }
