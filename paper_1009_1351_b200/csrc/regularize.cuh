@@ -28,8 +28,21 @@
 // item of a row) gets its running sum D initialised to a huge finite value, which no sliding
 // update can change, so its weight is exactly 0 at no per-evaluation cost; candidate rows
 // outside the image are skipped warp-uniformly.
-// Weights are never stored (recomputing beats 2*W^2 floats per pixel of HBM traffic).
+//
+// Stored weights ("reusing this factor ... instead of recomputing").  The weights
+// belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 the first sweep
+// (STORE_W = true) also writes every unnormalised weight as fp16 into
+// wts[image][side][band][tile_x][delta][RB rows][128 columns] -- one contiguous chunk per warp
+// band, written and later read as a sequential stream (DRAM-page friendly; a plane-per-offset
+// layout scatters 256-byte pieces and ran 3x slower) -- scaled so that the delta = 0 weight is 1
+// (margin 0); a side
+// whose sum reaches 6e4 (some weight near the fp16 maximum) takes the exact route, which stores
+// minimum-subtracted weights <= 1 instead.  Sweeps 2..M2 are gj_apply_kernel: a streaming pass
+// over the chunks, bound by HBM (2 bytes per weight) instead of by the FP32 pipes.  With M2 = 1
+// nothing is stored.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "common.cuh"
 
 namespace tnlm {
@@ -37,7 +50,6 @@ namespace tnlm {
 constexpr int SW_C = 4;        // columns per lane
 constexpr int SW_G = 4;        // search offsets (consecutive dc) per item
 constexpr int SW_TW = 128;     // tile width = 32 lanes x SW_C
-constexpr float SW_MARGIN = 90.0f;
 // Keeps ptxas from hoisting the next row's shared-memory loads over a whole march step (the
 // hoisted values push the kernel over 255 registers and spill); the other warp of the scheduler
 // covers the exposed load latency.
@@ -51,11 +63,15 @@ struct SweepParams {
     int ngroups;            // ceil(window / SW_G)
     int nb;                 // row bands per CTA; a CTA has 2*nb warps (band x side)
     int tiles_x, tiles_y;   // tiles per image
+    int rb;                 // rows per band (= RB of the sweep kernel that stored the weights)
+    int nbands;             // row bands per image in the stored-weight layout (tiles_y * nb of that sweep)
     float neg_c;            // -log2(e)/h^2
     float pos_c;            // +log2(e)/h^2
     float c_self;           // 1/(1+mu)
     float c_nb;             // mu/(2mu+2)
     float big_d;            // distance given to excluded candidates (finite, big_d*pos_c finite)
+    float margin;           // the delta = 0 weight is 2^-margin (90: compute only; 0: weights are stored)
+    float z_limit;          // a side whose weight sum is not below this is recomputed exactly
     int clip;               // apply max(.,0) to the output
 };
 
@@ -107,8 +123,10 @@ __device__ __forceinline__ void load_tile(float *__restrict__ dst, int rows, int
 template <int PB>
 __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, const float *__restrict__ sGj,
                                                const float *__restrict__ sUj, int GJW, int UJW, int pr, int pc,
-                                               int r, int c, int a, int ny, int nx, float neg_c, int lane)
+                                               int r, int c, int a, int ny, int nx, float neg_c, int lane,
+                                               __half *__restrict__ wpix, size_t wstride)
 {
+    // wpix (optional): slot of this pixel in offset 0 of its stored-weight chunk; offset stride wstride
     constexpr int GIW = SweepGeom<PB>::GIW;
     const int W = 2 * a + 1;
     float dmin = 3.0e38f;
@@ -116,7 +134,10 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
         float z = 0.f, aa = 0.f, dm = 3.0e38f;
         for (int idx = lane; idx < W * W; idx += 32) {
             const int dr = idx / W - a, dc = idx % W - a;
-            if ((unsigned)(r + dr) >= (unsigned)ny || (unsigned)(c + dc) >= (unsigned)nx) continue;
+            if ((unsigned)(r + dr) >= (unsigned)ny || (unsigned)(c + dc) >= (unsigned)nx) {
+                if (pass == 1 && wpix) wpix[(size_t)idx * wstride] = __float2half_rn(0.f);
+                continue;
+            }
             float D = 0.f;
             for (int y = 0; y <= 2 * PB; ++y)
                 for (int x = 0; x <= 2 * PB; ++x) {
@@ -126,7 +147,12 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
             if (pass == 0) {
                 dm = fminf(dm, D);
             } else {
-                const float e = exp2f(neg_c * (D - dmin));
+                float e = exp2f(neg_c * (D - dmin));
+                if (wpix) {                        // the sweeps that follow see exactly the stored value
+                    const __half eh = __float2half_rn(e);
+                    wpix[(size_t)idx * wstride] = eh;
+                    e = __half2float(eh);
+                }
                 z += e;
                 aa = fmaf(e, sUj[(pr + dr + a) * UJW + pc + dc + a], aa);
             }
@@ -146,9 +172,10 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
 
 // One Gauss-Jacobi sweep of Eq. (7) for every pixel of every phase of every slice.
 // grid.x = (S*N) * tiles_y * tiles_x; block = 64 * nb threads; warp w: band = w >> 1, side = w & 1.
-template <int PB, int RB>
+template <int PB, int RB, bool STORE_W>
 __global__ void __launch_bounds__(256, 1)
-gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out)
+gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
+                __half *__restrict__ wts)
 {
     using GEO = SweepGeom<PB>;
     constexpr int C = SW_C, G = SW_G, NGI = GEO::NGI, NGJ = GEO::NGJ, NUJ = GEO::NUJ, GIW = GEO::GIW;
@@ -221,7 +248,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             for (int c = 0; c < C; ++c) {
                 D0[c] += H[c];
                 if (s >= 2 * PB) {
-                    myK[(s - 2 * PB) * SW_TW + C * lane + c] = fmaf(D0[c], p.pos_c, -SW_MARGIN);
+                    myK[(s - 2 * PB) * SW_TW + C * lane + c] = fmaf(D0[c], p.pos_c, -p.margin);
                     D0[c] -= (PB > 0) ? ring[c][s % RING] : H[c];
                 }
                 ring[c][s % RING] = H[c];
@@ -237,12 +264,21 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 #pragma unroll
         for (int c = 0; c < C; ++c) { Z[rr][c] = 0.f; A[rr][c] = 0.f; }
 
+    // stored-weight chunk of this warp: [W*W][RB][128] halves
+    constexpr size_t WSTRIDE = (size_t)RB * SW_TW;         // halves per offset
+    __half *__restrict__ wchunk = nullptr;
+    if (STORE_W) {
+        const size_t gband = (size_t)(tile_r0 / RB) + band, tx = tile_c0 / SW_TW;
+        wchunk = wts + ((((size_t)img * 2 + side) * p.nbands + gband) * p.tiles_x + tx) *
+                           (size_t)((2 * a + 1) * (2 * a + 1)) * WSTRIDE;
+    }
+
     for (int dr = -a; dr <= a; ++dr) {
         unsigned okmask = 0;                       // pixel row and candidate row inside the image
 #pragma unroll
         for (int rr = 0; rr < RB; ++rr)
             if (r0 + rr < ny && (unsigned)(r0 + rr + dr) < (unsigned)ny) okmask |= 1u << rr;
-        if (okmask == 0) continue;
+        if (!STORE_W && okmask == 0) continue;     // (stored planes must be written even when all-zero)
         for (int dcg = 0; dcg < ng; ++dcg) {
             const int dc0 = -a + G * dcg;
             float D[G][C], ring[G][C][RING];
@@ -257,6 +293,8 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             const float4 *__restrict__ gjp = reinterpret_cast<const float4 *>(myGj + (lr0 + dr + a) * GJW) + lane + dcg;
             const float4 *__restrict__ ujp = reinterpret_cast<const float4 *>(myUj + (lr0 + dr + a) * UJW) + lane + dcg;
             const float4 *__restrict__ kp = reinterpret_cast<const float4 *>(myK) + lane;
+            __half *__restrict__ witem =
+                STORE_W ? wchunk + ((size_t)(dr + a) * (2 * a + 1) + (dc0 + a)) * WSTRIDE + C * lane : nullptr;
 #pragma unroll
             for (int s = 0; s < RB + 2 * PB; ++s) {
                 float gi_[4 * NGI], gj_[4 * NGJ];
@@ -301,16 +339,31 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         H[c] = h;
                     }
 #pragma unroll
+                    float e_[C];
+#pragma unroll
                     for (int c = 0; c < C; ++c) {
                         D[gg][c] += H[c];
                         if (s >= 2 * PB) {
                             const int rr = s - 2 * PB;
-                            const float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
+                            float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
+                            if (STORE_W) {         // accumulate exactly what the later sweeps will read
+                                e_[c] = e;
+                                e = __half2float(__float2half_rn(e));
+                            }
                             Z[rr][c] += e;
                             A[rr][c] = fmaf(e, uj_[c + gg], A[rr][c]);
                             D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[c];
                         }
                         ring[gg][c][s % RING] = H[c];
+                    }
+                    if (STORE_W && s >= 2 * PB) {  // one predicated 8-byte store: 4 fp16 weights of row rr, offset gg
+                        const int rr = s - 2 * PB;
+                        const __half2 lo = __floats2half2_rn(e_[0], e_[1]), hi = __floats2half2_rn(e_[2], e_[3]);
+                        uint2 pk;
+                        pk.x = *reinterpret_cast<const unsigned *>(&lo);
+                        pk.y = *reinterpret_cast<const unsigned *>(&hi);
+                        if (dc0 + gg <= a)         // (rows / columns past the image edge land in chunk padding)
+                            *reinterpret_cast<uint2 *>(witem + gg * WSTRIDE + rr * SW_TW) = pk;
                     }
                 }
                 SW_STEP_FENCE();
@@ -324,14 +377,16 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             const bool valid = (r0 + rr < ny) && (c0 + c < nx);
-            const bool bad = valid && !(Z[rr][c] < 1.0e38f);
+            const bool bad = valid && !(Z[rr][c] < p.z_limit);
             A[rr][c] = A[rr][c] / Z[rr][c];
             unsigned m = __ballot_sync(0xffffffffu, bad);
             while (m) {
                 const int L = __ffs(m) - 1;
                 m &= m - 1;
+                __half *wpix = STORE_W ? wchunk + rr * SW_TW + C * L + c : nullptr;
+                __syncwarp();                      // the fast path's stores to this pixel come first
                 const float v = exact_side_ratio<PB>(sGi, myGj, myUj, GJW, UJW, lr0 + rr, C * L + c, r0 + rr,
-                                                     tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane);
+                                                     tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane, wpix, WSTRIDE);
                 if (lane == L) A[rr][c] = v;
             }
         }
@@ -369,6 +424,106 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             }
         }
     }
+}
+
+// Sweeps 2..M2 with the stored weights: u_i'(x) = g_i(x)/(1+mu) + mu/(2mu+2) * sum over the two sides of
+// (sum_delta w u_j(x+delta)) / (sum_delta w), w read back as fp16 (2 bytes per weight: HBM bound).
+// CTA = one stored band: p.rb warps (one per row) x 32 lanes, lane l owns columns 4l..4l+3 of the
+// 128-column tile, so the CTA streams its two chunks front to back; u_j of both neighbours is
+// staged with its halo in shared memory, zero-filled outside the image (excluded candidates
+// carry weight 0 in the chunks).  grid.x = (S*N) * ceil(ny / rb) * tiles_x.
+__global__ void __launch_bounds__(320)
+gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
+                const __half *__restrict__ wts)
+{
+    constexpr int C = SW_C;
+    const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1;
+    const int nchunk = (W + 3) >> 2;
+    const int UW = 124 + 4 * (nchunk + 1);          // lane reads words [4l + 4k, 4l + 4k + 8)
+    const int rb = p.rb, urows = rb + 2 * a;
+    extern __shared__ float4 smem4[];
+    float *sU = reinterpret_cast<float *>(smem4);   // [2][urows][UW], origin (tile_r0 - a, tile_c0 - a)
+
+    const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
+    const int img = blockIdx.x / tiles_per_img;
+    const int tl = blockIdx.x - img * tiles_per_img;
+    const int gband = tl / p.tiles_x, tx = tl - gband * p.tiles_x;
+    const int tile_r0 = gband * rb, tile_c0 = tx * SW_TW;
+    const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
+    const size_t npix = (size_t)nx * ny;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
+        load_tile(sU + s * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a,
+                  tile_c0 - a, ny, nx, warp, rb, lane);
+    }
+    __syncthreads();
+
+    const int r = tile_r0 + warp, c0 = tile_c0 + C * lane;
+    if (r >= ny || c0 >= nx) return;
+    const size_t wstride = (size_t)rb * SW_TW;                             // halves per offset
+    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)(W * W) * wstride;
+    const __half *__restrict__ wp = wts + ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)(W * W) * wstride +
+                                    warp * SW_TW + C * lane;
+    float Z[2][C], A[2][C];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int c = 0; c < C; ++c) { Z[s][c] = 0.f; A[s][c] = 0.f; }
+
+    {
+        // 4 offsets x 2 sides = 8 independent 8-byte loads in flight per thread and chunk
+        for (int dr = 0; dr < W; ++dr) {
+            const float4 *__restrict__ up0 = reinterpret_cast<const float4 *>(sU + (warp + dr) * UW) + lane;
+            const float4 *__restrict__ up1 = reinterpret_cast<const float4 *>(sU + (urows + warp + dr) * UW) + lane;
+            const __half *__restrict__ wrow = wp + (size_t)dr * W * wstride;
+#pragma unroll 2
+            for (int k = 0; k < nchunk; ++k) {
+                uint2 wv[2][4];
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const int dc = min(4 * k + jj, W - 1);     // the tail re-reads the last plane, unused
+                    const __half *__restrict__ q = wrow + (size_t)dc * wstride;
+                    wv[0][jj] = __ldg(reinterpret_cast<const uint2 *>(q));
+                    wv[1][jj] = __ldg(reinterpret_cast<const uint2 *>(q + side_stride));
+                }
+                float uw[2][8];
+                {
+                    const float4 a0 = up0[k], a1 = up0[k + 1], b0 = up1[k], b1 = up1[k + 1];
+                    uw[0][0] = a0.x; uw[0][1] = a0.y; uw[0][2] = a0.z; uw[0][3] = a0.w;
+                    uw[0][4] = a1.x; uw[0][5] = a1.y; uw[0][6] = a1.z; uw[0][7] = a1.w;
+                    uw[1][0] = b0.x; uw[1][1] = b0.y; uw[1][2] = b0.z; uw[1][3] = b0.w;
+                    uw[1][4] = b1.x; uw[1][5] = b1.y; uw[1][6] = b1.z; uw[1][7] = b1.w;
+                }
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    if (4 * k + jj < W) {
+#pragma unroll
+                        for (int s = 0; s < 2; ++s) {
+                            const float2 lo = __half22float2(*reinterpret_cast<const __half2 *>(&wv[s][jj].x));
+                            const float2 hi = __half22float2(*reinterpret_cast<const __half2 *>(&wv[s][jj].y));
+                            const float w[C] = {lo.x, lo.y, hi.x, hi.y};
+#pragma unroll
+                            for (int c = 0; c < C; ++c) {
+                                Z[s][c] += w[c];
+                                A[s][c] = fmaf(w[c], uw[s][c + jj], A[s][c]);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+    const float *__restrict__ gi = g + (size_t)img * npix + (size_t)r * nx + c0;
+    float *__restrict__ o = out + (size_t)img * npix + (size_t)r * nx + c0;
+#pragma unroll
+    for (int c = 0; c < C; ++c)
+        if (c0 + c < nx) {
+            float v = fmaf(p.c_nb, A[0][c] / Z[0][c] + A[1][c] / Z[1][c], p.c_self * __ldg(gi + c));
+            if (p.clip) v = fmaxf(v, 0.f);
+            o[c] = v;
+        }
 }
 
 // f = max(g, 0): the m2 = 0 case of steps 3-5.

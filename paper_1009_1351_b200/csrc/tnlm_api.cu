@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -21,7 +22,8 @@ static constexpr int MAX_PATCH = 9, MAX_WINDOW = 31;
 
 // One compiled shape of gj_sweep_kernel<PB, RB> with nb row bands per CTA (regularize.cuh).
 struct SweepShape {
-    const void *fn = nullptr;
+    const void *fn = nullptr;       // compute only
+    const void *fn_store = nullptr; // compute and store the weights (first of several sweeps)
     int rb = 0, nb = 0, occ = 0;    // rows per band, bands per CTA, resident CTAs per SM
     size_t smem = 0;
 };
@@ -44,6 +46,9 @@ struct tnlm_handle {
     float *d_ua = nullptr, *d_ub = nullptr;                                  // sweep ping-pong
     float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr;                   // sinograms
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
+    __half *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
+    size_t wts_cap = 0;               // in halves
+    size_t apply_smem = 0;
     double *d_scal = nullptr;
     int scal_cap = 0;
     long long launches = 0;
@@ -130,12 +135,13 @@ static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, st
 template <int PB, int RB>
 static cudaError_t add_sweep_shapes(tnlm_handle *H, size_t smem_limit)
 {
-    const void *fn = (const void *)gj_sweep_kernel<PB, RB>;
+    const void *fn = (const void *)gj_sweep_kernel<PB, RB, false>;
+    const void *fn_store = (const void *)gj_sweep_kernel<PB, RB, true>;
     size_t biggest = 0;
     std::vector<SweepShape> mine;
     for (int nb = 4; nb >= 1; nb >>= 1) {
         SweepShape sh;
-        sh.fn = fn; sh.rb = RB; sh.nb = nb;
+        sh.fn = fn; sh.fn_store = fn_store; sh.rb = RB; sh.nb = nb;
         sh.smem = SweepGeom<PB>::smem_words(H->R.a, H->R.ngroups, nb, RB) * sizeof(float);
         if (sh.smem > smem_limit) continue;
         if (sh.smem > biggest) biggest = sh.smem;
@@ -143,10 +149,14 @@ static cudaError_t add_sweep_shapes(tnlm_handle *H, size_t smem_limit)
     }
     if (mine.empty()) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)biggest);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_store, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)biggest);
     if (e != cudaSuccess) return e;
     for (SweepShape &sh : mine) {
+        int occ_store = 0;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&sh.occ, fn, 64 * sh.nb, sh.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_store, fn_store, 64 * sh.nb, sh.smem);
         if (e != cudaSuccess) return e;
+        sh.occ = std::min(sh.occ, occ_store);
         if (sh.occ >= 1) H->shapes.push_back(sh);
     }
     return cudaSuccess;
@@ -225,7 +235,16 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     R.c_self = (float)(1.0 / (1.0 + (double)mu));
     R.c_nb = (float)((double)mu / (2.0 * (double)mu + 2.0));
     R.big_d = (float)std::fmin(1e30, 1e37 / c);
+    R.margin = 90.0f;
+    R.z_limit = 1.0e38f;
     R.clip = 0;
+    {
+        const int nchunk = (window + 3) / 4;
+        H->apply_smem = (size_t)2 * (10 + 2 * R.a) * (124 + 4 * (nchunk + 1)) * sizeof(float);   // rb <= 10
+        ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)H->apply_smem);
+        if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
+    }
     H->n_sm = prop.multiProcessorCount;
     ce = build_sweep_shapes(H, (size_t)prop.sharedMemPerBlockOptin);
     if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "sweep kernel setup"); }
@@ -272,6 +291,7 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     if (!H) return TNLM_INVALID_ARG;
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
+    if (H->d_wts) cudaFree(H->d_wts);
     if (H->d_tab) cudaFree(H->d_tab);
     if (H->d_rng) cudaFree(H->d_rng);
     if (H->d_views) cudaFree(H->d_views);
@@ -398,28 +418,85 @@ extern "C" int tnlm_cgls_step(tnlm_handle *H, const float *f_in, const float *y,
 }
 
 // ------------------------------------------------------------------------------ TNLM
-static int launch_sweep(tnlm_handle *H, const float *g, const float *u, float *out, int clip, int n_slices, cudaStream_t st)
+// The cheapest launchable shape for n_img images (cost model above).
+static const SweepShape *pick_shape(tnlm_handle *H, int n_img)
 {
-    const int nimg = n_slices * H->n_phase;
     const SweepShape *best = nullptr;
     double best_cost = 0.0;
+    // tuning override for experiments: TNLM_SWEEP_SHAPE="rb,nb" restricts the choice
+    int want_rb = 0, want_nb = 0;
+    if (const char *ev = std::getenv("TNLM_SWEEP_SHAPE")) std::sscanf(ev, "%d,%d", &want_rb, &want_nb);
     for (const SweepShape &sh : H->shapes) {
-        const double c = sweep_cost(H, sh, nimg);
+        if ((want_rb && sh.rb != want_rb) || (want_nb && sh.nb != want_nb)) continue;
+        const double c = sweep_cost(H, sh, n_img);
         if (!best || c < best_cost) { best = &sh; best_cost = c; }
     }
-    SweepParams R = H->R;
-    R.clip = clip;
-    R.nb = best->nb;
-    const int th = best->nb * best->rb;
+    if (!best) fail(H, TNLM_INVALID_ARG, "TNLM_SWEEP_SHAPE names a shape that is not available");
+    return best;
+}
+
+static void fill_layout(const tnlm_handle *H, const SweepShape &sh, SweepParams &R)
+{
+    const int th = sh.nb * sh.rb;
+    R.nb = sh.nb;
+    R.rb = sh.rb;
     R.tiles_x = (H->nx + SW_TW - 1) / SW_TW;
     R.tiles_y = (H->ny + th - 1) / th;
+    R.nbands = R.tiles_y * sh.nb;
+}
+
+// One sweep with the weights computed on the fly; wts != NULL also stores them (fp16 chunks).
+static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
+                        int n_slices, __half *wts, cudaStream_t st)
+{
+    const int nimg = n_slices * H->n_phase;
+    SweepParams R = H->R;
+    R.clip = clip;
+    fill_layout(H, sh, R);
+    if (wts) { R.margin = 0.0f; R.z_limit = 6.0e4f; }   // stored weights: delta = 0 weighs 1, fp16 range
     const long long ctas = (long long)nimg * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
-    void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out};
-    cudaError_t e = cudaLaunchKernel(best->fn, dim3((unsigned)ctas), dim3(64 * best->nb), args, best->smem, st);
+    void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out, (void *)&wts};
+    cudaError_t e = cudaLaunchKernel(wts ? sh.fn_store : sh.fn, dim3((unsigned)ctas), dim3(64 * sh.nb), args, sh.smem, st);
     if (e != cudaSuccess) return cuda_fail(H, e, "cudaLaunchKernel(gj_sweep_kernel)");
     LAUNCHED(H);
     return TNLM_OK;
+}
+
+// One sweep with the stored weights of this outer iteration (written by shape sh).
+static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
+                        int n_slices, const __half *wts, cudaStream_t st)
+{
+    SweepParams R = H->R;
+    R.clip = clip;
+    fill_layout(H, sh, R);
+    R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
+    const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
+    if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
+    const size_t smem = (size_t)2 * (sh.rb + 2 * R.a) * (124 + 4 * ((H->window + 3) / 4 + 1)) * sizeof(float);
+    gj_apply_kernel<<<(unsigned)ctas, 32 * sh.rb, smem, st>>>(R, g, u, out, wts);
+    LAUNCHED(H);
+    return TNLM_OK;
+}
+
+// Weight storage for m2 > 1: 2 bytes x 2 sides x W^2 per pixel of the padded band/tile grid.
+// Returns NULL (recompute every sweep instead) when that exceeds the cap
+// (TNLM_WEIGHT_CACHE_MB, default 16384; 0 disables).
+static __half *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices)
+{
+    size_t cap_mb = 16384;
+    if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) cap_mb = (size_t)std::strtoull(ev, nullptr, 10);
+    SweepParams R = H->R;
+    fill_layout(H, sh, R);
+    const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
+    if (need * sizeof(__half) > cap_mb * 1048576ull) return nullptr;
+    if (need > H->wts_cap) {
+        if (H->d_wts) cudaFree(H->d_wts);
+        H->d_wts = nullptr; H->wts_cap = 0;
+        if (cudaMalloc(&H->d_wts, need * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        H->wts_cap = need;
+    }
+    return H->d_wts;
 }
 
 // g -> f_out; g and f_out are distinct device buffers or the same buffer.
@@ -438,12 +515,17 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
     const float *src = g;
     float *pp[2] = {H->d_ua, H->d_ub};
     int which = 0;
+    const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
+    if (!sh) return TNLM_INVALID_ARG;
+    __half *wts = (m2 > 1) ? weight_cache(H, *sh, n_slices) : nullptr;   // weights are those of g for all sweeps (L162)
     for (int m = 0; m < m2; ++m) {
         const bool last = (m + 1 == m2);
         float *dst;
         if (last && !alias) dst = f_out;
         else { dst = pp[which]; if (dst == src) { which ^= 1; dst = pp[which]; } }
-        if ((rc = launch_sweep(H, g, src, dst, last ? 1 : 0, n_slices, st))) return rc;
+        if (m == 0 || !wts) rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
+        else rc = launch_apply(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
+        if (rc) return rc;
         src = dst;
         which ^= 1;
     }

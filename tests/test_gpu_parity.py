@@ -218,6 +218,27 @@ def test_regularize_edge_cases(T):
     assert (out - cst).abs().max().item() < 1e-8
 
 
+def test_stored_weights_equal_recomputed_weights(T, monkeypatch):
+    # m2 > 1 stores the weights of g^(k) as fp16 planes in sweep 1 and streams them in sweeps 2..m2
+    # (PAPER.md:L162, L206); TNLM_WEIGHT_CACHE_MB=0 recomputes them in fp32 every sweep.  Both are the
+    # same iteration; moving edges (tumour) and a tiny h exercise the exact-route weights too.
+    torch, tn = T
+    for (N, ny, nx, W, d, h, mu, m2) in [(3, 70, 132, 11, 5, 0.008, 0.3, 4), (4, 41, 67, 5, 3, 0.002, 0.5, 3)]:
+        g = noisy_stack(N, ny, nx, seed=77)
+        gd = dev(torch, g)
+        hd = tn.create(None, nx, ny, N, W, d, h, mu)
+        a = torch.empty_like(gd); b = torch.empty_like(gd)
+        monkeypatch.setenv("TNLM_WEIGHT_CACHE_MB", "0")
+        n0 = hd.launch_count
+        tn.regularize_step(hd, gd, m2, a)
+        monkeypatch.delenv("TNLM_WEIGHT_CACHE_MB")
+        tn.regularize_step(hd, gd, m2, b)
+        want = oracle.regularize_step(g, W, d, h, mu, m2)
+        assert rel(a.cpu().numpy(), want) < STEP_TOL and rel(b.cpu().numpy(), want) < STEP_TOL
+        assert rel(b.cpu().numpy(), a.cpu().numpy()) < 2e-5
+        assert np.abs(b.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
+
+
 def test_regularize_multi_slice_equals_per_slice(T):
     torch, tn = T
     N, ny, nx, S = 3, 40, 72, 3
