@@ -31,17 +31,19 @@
 //
 // Stored weights ("reusing this factor ... instead of recomputing").  The weights
 // belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 the first sweep
-// (STORE_W = true) also writes every unnormalised weight as fp16 into
+// (STORE_W = true) also writes every unnormalised weight as bf16 into
 // wts[image][side][band][tile_x][delta][RB rows][128 columns] -- one contiguous chunk per warp
 // band, written and later read as a sequential stream (DRAM-page friendly; a plane-per-offset
-// layout scatters 256-byte pieces and ran 3x slower) -- scaled so that the delta = 0 weight is 1
-// (margin 0); a side
-// whose sum reaches 6e4 (some weight near the fp16 maximum) takes the exact route, which stores
-// minimum-subtracted weights <= 1 instead.  Sweeps 2..M2 are gj_apply_kernel: a streaming pass
+// layout scatters 256-byte pieces and ran 3x slower).  bf16 keeps the fp32 exponent range, so the
+// stored values are the very 2^(c(D0-D)-90) of the fast path (an fp16 version needed its own
+// reference and sent every moving edge through the slow exact route: 2.6x slower); the quotient
+// A/Z of Eq. (7) does not depend on the per-pixel scale, and the 2^-9 rounding of each weight
+// moves it by < 1e-6 relative.  Pixels on the exact route store their
+// minimum-subtracted weights instead.  Sweeps 2..M2 are gj_apply_kernel: a streaming pass
 // over the chunks, bound by HBM (2 bytes per weight) instead of by the FP32 pipes.  With M2 = 1
 // nothing is stored.
 #pragma once
-#include <cuda_fp16.h>
+#include <cuda_bf16.h>
 
 #include "common.cuh"
 
@@ -70,7 +72,7 @@ struct SweepParams {
     float c_self;           // 1/(1+mu)
     float c_nb;             // mu/(2mu+2)
     float big_d;            // distance given to excluded candidates (finite, big_d*pos_c finite)
-    float margin;           // the delta = 0 weight is 2^-margin (90: compute only; 0: weights are stored)
+    float margin;           // the delta = 0 weight is 2^-margin (90)
     float z_limit;          // a side whose weight sum is not below this is recomputed exactly
     int clip;               // apply max(.,0) to the output
 };
@@ -124,7 +126,7 @@ template <int PB>
 __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, const float *__restrict__ sGj,
                                                const float *__restrict__ sUj, int GJW, int UJW, int pr, int pc,
                                                int r, int c, int a, int ny, int nx, float neg_c, int lane,
-                                               __half *__restrict__ wpix, size_t wstride)
+                                               __nv_bfloat16 *__restrict__ wpix, size_t wstride)
 {
     // wpix (optional): slot of this pixel in offset 0 of its stored-weight chunk; offset stride wstride
     constexpr int GIW = SweepGeom<PB>::GIW;
@@ -135,7 +137,7 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
         for (int idx = lane; idx < W * W; idx += 32) {
             const int dr = idx / W - a, dc = idx % W - a;
             if ((unsigned)(r + dr) >= (unsigned)ny || (unsigned)(c + dc) >= (unsigned)nx) {
-                if (pass == 1 && wpix) wpix[(size_t)idx * wstride] = __float2half_rn(0.f);
+                if (pass == 1 && wpix) wpix[(size_t)idx * wstride] = __float2bfloat16_rn(0.f);
                 continue;
             }
             float D = 0.f;
@@ -149,9 +151,9 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
             } else {
                 float e = exp2f(neg_c * (D - dmin));
                 if (wpix) {                        // the sweeps that follow see exactly the stored value
-                    const __half eh = __float2half_rn(e);
+                    const __nv_bfloat16 eh = __float2bfloat16_rn(e);
                     wpix[(size_t)idx * wstride] = eh;
-                    e = __half2float(eh);
+                    e = __bfloat162float(eh);
                 }
                 z += e;
                 aa = fmaf(e, sUj[(pr + dr + a) * UJW + pc + dc + a], aa);
@@ -175,7 +177,7 @@ __device__ __noinline__ float exact_side_ratio(const float *__restrict__ sGi, co
 template <int PB, int RB, bool STORE_W>
 __global__ void __launch_bounds__(256, 1)
 gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
-                __half *__restrict__ wts)
+                __nv_bfloat16 *__restrict__ wts)
 {
     using GEO = SweepGeom<PB>;
     constexpr int C = SW_C, G = SW_G, NGI = GEO::NGI, NGJ = GEO::NGJ, NUJ = GEO::NUJ, GIW = GEO::GIW;
@@ -266,7 +268,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 
     // stored-weight chunk of this warp: [W*W][RB][128] halves
     constexpr size_t WSTRIDE = (size_t)RB * SW_TW;         // halves per offset
-    __half *__restrict__ wchunk = nullptr;
+    __nv_bfloat16 *__restrict__ wchunk = nullptr;
     if (STORE_W) {
         const size_t gband = (size_t)(tile_r0 / RB) + band, tx = tile_c0 / SW_TW;
         wchunk = wts + ((((size_t)img * 2 + side) * p.nbands + gband) * p.tiles_x + tx) *
@@ -293,7 +295,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             const float4 *__restrict__ gjp = reinterpret_cast<const float4 *>(myGj + (lr0 + dr + a) * GJW) + lane + dcg;
             const float4 *__restrict__ ujp = reinterpret_cast<const float4 *>(myUj + (lr0 + dr + a) * UJW) + lane + dcg;
             const float4 *__restrict__ kp = reinterpret_cast<const float4 *>(myK) + lane;
-            __half *__restrict__ witem =
+            __nv_bfloat16 *__restrict__ witem =
                 STORE_W ? wchunk + ((size_t)(dr + a) * (2 * a + 1) + (dc0 + a)) * WSTRIDE + C * lane : nullptr;
 #pragma unroll
             for (int s = 0; s < RB + 2 * PB; ++s) {
@@ -345,20 +347,17 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         D[gg][c] += H[c];
                         if (s >= 2 * PB) {
                             const int rr = s - 2 * PB;
-                            float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
-                            if (STORE_W) {         // accumulate exactly what the later sweeps will read
-                                e_[c] = e;
-                                e = __half2float(__float2half_rn(e));
-                            }
+                            const float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
+                            if (STORE_W) e_[c] = e;
                             Z[rr][c] += e;
                             A[rr][c] = fmaf(e, uj_[c + gg], A[rr][c]);
                             D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[c];
                         }
                         ring[gg][c][s % RING] = H[c];
                     }
-                    if (STORE_W && s >= 2 * PB) {  // one predicated 8-byte store: 4 fp16 weights of row rr, offset gg
+                    if (STORE_W && s >= 2 * PB) {  // one predicated 8-byte store: 4 bf16 weights of row rr, offset gg
                         const int rr = s - 2 * PB;
-                        const __half2 lo = __floats2half2_rn(e_[0], e_[1]), hi = __floats2half2_rn(e_[2], e_[3]);
+                        const __nv_bfloat162 lo = __floats2bfloat162_rn(e_[0], e_[1]), hi = __floats2bfloat162_rn(e_[2], e_[3]);
                         uint2 pk;
                         pk.x = *reinterpret_cast<const unsigned *>(&lo);
                         pk.y = *reinterpret_cast<const unsigned *>(&hi);
@@ -383,7 +382,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             while (m) {
                 const int L = __ffs(m) - 1;
                 m &= m - 1;
-                __half *wpix = STORE_W ? wchunk + rr * SW_TW + C * L + c : nullptr;
+                __nv_bfloat16 *wpix = STORE_W ? wchunk + rr * SW_TW + C * L + c : nullptr;
                 __syncwarp();                      // the fast path's stores to this pixel come first
                 const float v = exact_side_ratio<PB>(sGi, myGj, myUj, GJW, UJW, lr0 + rr, C * L + c, r0 + rr,
                                                      tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane, wpix, WSTRIDE);
@@ -426,23 +425,74 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     }
 }
 
+// ---- mbarrier / bulk-copy (TMA) primitives used by gj_apply_kernel -----------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared bulk copy (16-byte aligned, size a multiple of 16), completion counted on bar
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
 // Sweeps 2..M2 with the stored weights: u_i'(x) = g_i(x)/(1+mu) + mu/(2mu+2) * sum over the two sides of
-// (sum_delta w u_j(x+delta)) / (sum_delta w), w read back as fp16 (2 bytes per weight: HBM bound).
-// CTA = one stored band: p.rb warps (one per row) x 32 lanes, lane l owns columns 4l..4l+3 of the
-// 128-column tile, so the CTA streams its two chunks front to back; u_j of both neighbours is
-// staged with its halo in shared memory, zero-filled outside the image (excluded candidates
-// carry weight 0 in the chunks).  grid.x = (S*N) * ceil(ny / rb) * tiles_x.
-__global__ void __launch_bounds__(320)
+// (sum_delta w u_j(x+delta)) / (sum_delta w), w read back as bf16 (2 bytes per weight: HBM bound).
+// CTA = one stored band: p.rb consumer warps (one per row, lane l owns columns 4l..4l+3 of the
+// 128-column tile) + one producer warp.  The band's two chunks are contiguous in memory, so the
+// producer streams them front to back with bulk copies (cp.async.bulk, TMA) of up to AP_SO
+// offsets per stage into an AP_NS-deep shared-memory ring; full/empty mbarriers hand stages
+// over, nothing else synchronises.  u_j of both neighbours is staged with its halo in shared
+// memory, zero-filled outside the image (excluded candidates carry weight 0 in the chunks).
+// grid.x = (S*N) * ceil(ny / rb) * tiles_x; block = 32 * (rb + 1).
+constexpr int AP_SO = 4;     // offsets (consecutive dc of one dr) per stage
+constexpr int AP_NS = 4;     // stages in flight
+__host__ __device__ inline int apply_uw(int window) { return 124 + 4 * ((window + 3) / 4 + 1); }
+__host__ __device__ inline size_t apply_smem_bytes(int window, int rb)
+{
+    const int a = (window - 1) / 2;
+    return (size_t)AP_NS * AP_SO * rb * SW_TW * sizeof(__nv_bfloat16) + (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) +
+           2 * AP_NS * sizeof(uint64_t);
+}
+
+__global__ void __launch_bounds__(352)
 gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
-                const __half *__restrict__ wts)
+                const __nv_bfloat16 *__restrict__ wts)
 {
     constexpr int C = SW_C;
     const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1;
     const int nchunk = (W + 3) >> 2;
-    const int UW = 124 + 4 * (nchunk + 1);          // lane reads words [4l + 4k, 4l + 4k + 8)
+    const int UW = apply_uw(W);                     // lane reads words [4l + 4k, 4l + 4k + 8)
     const int rb = p.rb, urows = rb + 2 * a;
+    const size_t wstride = (size_t)rb * SW_TW;      // halves per offset
     extern __shared__ float4 smem4[];
-    float *sU = reinterpret_cast<float *>(smem4);   // [2][urows][UW], origin (tile_r0 - a, tile_c0 - a)
+    __nv_bfloat16 *sW = reinterpret_cast<__nv_bfloat16 *>(smem4);                                 // [AP_NS][AP_SO][rb][128]
+    float *sU = reinterpret_cast<float *>(sW + (size_t)AP_NS * AP_SO * wstride);    // [2][urows][UW]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sU + 2 * urows * UW);             // [AP_NS], then empty[AP_NS]
+    uint64_t *empty = full + AP_NS;
 
     const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
     const int img = blockIdx.x / tiles_per_img;
@@ -452,75 +502,92 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
     const size_t npix = (size_t)nx * ny;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < AP_NS; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, rb); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    // stage t = (side, dr, k): offsets dr*W + 4k .. of that side's chunk, min(4, W-4k) of them
+    const int stages_per_side = W * nchunk, T = 2 * stages_per_side;
+    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)(W * W) * wstride;
+    const __nv_bfloat16 *__restrict__ chunk0 = wts + ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)(W * W) * wstride;
+
+    if (warp == rb) {                               // ---- producer warp: one lane issues the bulk copies
+        if (lane == 0) {
+            for (int t = 0; t < T; ++t) {
+                const int slot = t % AP_NS;
+                if (t >= AP_NS) mbar_wait(empty + slot, ((t / AP_NS) - 1) & 1);
+                const int sd = t / stages_per_side, rem = t - sd * stages_per_side;
+                const int dr = rem / nchunk, k = rem - dr * nchunk;
+                const int noff = min(AP_SO, W - AP_SO * k);
+                const unsigned bytes = (unsigned)(noff * wstride * sizeof(__nv_bfloat16));
+                mbar_expect_tx(full + slot, bytes);
+                bulk_g2s(sW + (size_t)slot * AP_SO * wstride, chunk0 + sd * side_stride + (size_t)(dr * W + AP_SO * k) * wstride,
+                         bytes, full + slot);
+            }
+        }
+        return;
+    }
+
+    // ---- consumer warps: stage u_j (overlaps the first bulk copies), then drain the ring
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
         const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
         load_tile(sU + s * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a,
                   tile_c0 - a, ny, nx, warp, rb, lane);
     }
-    __syncthreads();
+    asm volatile("bar.sync 1, %0;" ::"r"(32 * rb) : "memory");      // consumers only
 
     const int r = tile_r0 + warp, c0 = tile_c0 + C * lane;
-    if (r >= ny || c0 >= nx) return;
-    const size_t wstride = (size_t)rb * SW_TW;                             // halves per offset
-    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)(W * W) * wstride;
-    const __half *__restrict__ wp = wts + ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)(W * W) * wstride +
-                                    warp * SW_TW + C * lane;
-    float Z[2][C], A[2][C];
-#pragma unroll
-    for (int s = 0; s < 2; ++s)
-#pragma unroll
-        for (int c = 0; c < C; ++c) { Z[s][c] = 0.f; A[s][c] = 0.f; }
-
-    {
-        // 4 offsets x 2 sides = 8 independent 8-byte loads in flight per thread and chunk
+    float nbsum[C] = {0.f, 0.f, 0.f, 0.f};
+    int t = 0;
+#pragma unroll 1
+    for (int s = 0; s < 2; ++s) {
+        float Z[C] = {0.f, 0.f, 0.f, 0.f}, A[C] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 1
         for (int dr = 0; dr < W; ++dr) {
-            const float4 *__restrict__ up0 = reinterpret_cast<const float4 *>(sU + (warp + dr) * UW) + lane;
-            const float4 *__restrict__ up1 = reinterpret_cast<const float4 *>(sU + (urows + warp + dr) * UW) + lane;
-            const __half *__restrict__ wrow = wp + (size_t)dr * W * wstride;
-#pragma unroll 2
-            for (int k = 0; k < nchunk; ++k) {
-                uint2 wv[2][4];
+            const float4 *__restrict__ up = reinterpret_cast<const float4 *>(sU + (s * urows + warp + dr) * UW) + lane;
+#pragma unroll 1
+            for (int k = 0; k < nchunk; ++k, ++t) {
+                const int slot = t % AP_NS;
+                const float4 u0 = up[k], u1 = up[k + 1];
+                const float uw[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
+                const int noff = min(AP_SO, W - AP_SO * k);
+                mbar_wait(full + slot, (t / AP_NS) & 1);
+                const uint2 *__restrict__ wq = reinterpret_cast<const uint2 *>(sW + (size_t)slot * AP_SO * wstride + warp * SW_TW) + lane;
+                uint2 wv[AP_SO];
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    const int dc = min(4 * k + jj, W - 1);     // the tail re-reads the last plane, unused
-                    const __half *__restrict__ q = wrow + (size_t)dc * wstride;
-                    wv[0][jj] = __ldg(reinterpret_cast<const uint2 *>(q));
-                    wv[1][jj] = __ldg(reinterpret_cast<const uint2 *>(q + side_stride));
-                }
-                float uw[2][8];
-                {
-                    const float4 a0 = up0[k], a1 = up0[k + 1], b0 = up1[k], b1 = up1[k + 1];
-                    uw[0][0] = a0.x; uw[0][1] = a0.y; uw[0][2] = a0.z; uw[0][3] = a0.w;
-                    uw[0][4] = a1.x; uw[0][5] = a1.y; uw[0][6] = a1.z; uw[0][7] = a1.w;
-                    uw[1][0] = b0.x; uw[1][1] = b0.y; uw[1][2] = b0.z; uw[1][3] = b0.w;
-                    uw[1][4] = b1.x; uw[1][5] = b1.y; uw[1][6] = b1.z; uw[1][7] = b1.w;
-                }
+                for (int jj = 0; jj < AP_SO; ++jj) wv[jj] = wq[(jj < noff ? jj : 0) * (wstride / 4)];
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + slot);           // values are in registers: slot is free
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    if (4 * k + jj < W) {
+                for (int jj = 0; jj < AP_SO; ++jj) {
+                    if (jj < noff) {
+                        const float2 lo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&wv[jj].x));
+                        const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&wv[jj].y));
+                        const float w[C] = {lo.x, lo.y, hi.x, hi.y};
 #pragma unroll
-                        for (int s = 0; s < 2; ++s) {
-                            const float2 lo = __half22float2(*reinterpret_cast<const __half2 *>(&wv[s][jj].x));
-                            const float2 hi = __half22float2(*reinterpret_cast<const __half2 *>(&wv[s][jj].y));
-                            const float w[C] = {lo.x, lo.y, hi.x, hi.y};
-#pragma unroll
-                            for (int c = 0; c < C; ++c) {
-                                Z[s][c] += w[c];
-                                A[s][c] = fmaf(w[c], uw[s][c + jj], A[s][c]);
-                            }
+                        for (int c = 0; c < C; ++c) {
+                            Z[c] += w[c];
+                            A[c] = fmaf(w[c], uw[c + jj], A[c]);
                         }
                     }
                 }
             }
         }
+#pragma unroll
+        for (int c = 0; c < C; ++c) nbsum[c] += A[c] / Z[c];
     }
+    if (r >= ny || c0 >= nx) return;
     const float *__restrict__ gi = g + (size_t)img * npix + (size_t)r * nx + c0;
     float *__restrict__ o = out + (size_t)img * npix + (size_t)r * nx + c0;
 #pragma unroll
     for (int c = 0; c < C; ++c)
         if (c0 + c < nx) {
-            float v = fmaf(p.c_nb, A[0][c] / Z[0][c] + A[1][c] / Z[1][c], p.c_self * __ldg(gi + c));
+            float v = fmaf(p.c_nb, nbsum[c], p.c_self * __ldg(gi + c));
             if (p.clip) v = fmaxf(v, 0.f);
             o[c] = v;
         }

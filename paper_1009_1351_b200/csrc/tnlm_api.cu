@@ -46,7 +46,7 @@ struct tnlm_handle {
     float *d_ua = nullptr, *d_ub = nullptr;                                  // sweep ping-pong
     float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr;                   // sinograms
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
-    __half *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
+    __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
     size_t wts_cap = 0;               // in halves
     size_t apply_smem = 0;
     double *d_scal = nullptr;
@@ -239,8 +239,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     R.z_limit = 1.0e38f;
     R.clip = 0;
     {
-        const int nchunk = (window + 3) / 4;
-        H->apply_smem = (size_t)2 * (10 + 2 * R.a) * (124 + 4 * (nchunk + 1)) * sizeof(float);   // rb <= 10
+        H->apply_smem = apply_smem_bytes(window, 10);   // rb <= 10
         ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)H->apply_smem);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
@@ -445,15 +444,14 @@ static void fill_layout(const tnlm_handle *H, const SweepShape &sh, SweepParams 
     R.nbands = R.tiles_y * sh.nb;
 }
 
-// One sweep with the weights computed on the fly; wts != NULL also stores them (fp16 chunks).
+// One sweep with the weights computed on the fly; wts != NULL also stores them (bf16 chunks).
 static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
-                        int n_slices, __half *wts, cudaStream_t st)
+                        int n_slices, __nv_bfloat16 *wts, cudaStream_t st)
 {
     const int nimg = n_slices * H->n_phase;
     SweepParams R = H->R;
     R.clip = clip;
     fill_layout(H, sh, R);
-    if (wts) { R.margin = 0.0f; R.z_limit = 6.0e4f; }   // stored weights: delta = 0 weighs 1, fp16 range
     const long long ctas = (long long)nimg * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
     void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out, (void *)&wts};
@@ -465,7 +463,7 @@ static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, co
 
 // One sweep with the stored weights of this outer iteration (written by shape sh).
 static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
-                        int n_slices, const __half *wts, cudaStream_t st)
+                        int n_slices, const __nv_bfloat16 *wts, cudaStream_t st)
 {
     SweepParams R = H->R;
     R.clip = clip;
@@ -473,8 +471,7 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
-    const size_t smem = (size_t)2 * (sh.rb + 2 * R.a) * (124 + 4 * ((H->window + 3) / 4 + 1)) * sizeof(float);
-    gj_apply_kernel<<<(unsigned)ctas, 32 * sh.rb, smem, st>>>(R, g, u, out, wts);
+    gj_apply_kernel<<<(unsigned)ctas, 32 * (sh.rb + 1), apply_smem_bytes(H->window, sh.rb), st>>>(R, g, u, out, wts);
     LAUNCHED(H);
     return TNLM_OK;
 }
@@ -482,18 +479,18 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
 // Weight storage for m2 > 1: 2 bytes x 2 sides x W^2 per pixel of the padded band/tile grid.
 // Returns NULL (recompute every sweep instead) when that exceeds the cap
 // (TNLM_WEIGHT_CACHE_MB, default 16384; 0 disables).
-static __half *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices)
+static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices)
 {
     size_t cap_mb = 16384;
     if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) cap_mb = (size_t)std::strtoull(ev, nullptr, 10);
     SweepParams R = H->R;
     fill_layout(H, sh, R);
     const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
-    if (need * sizeof(__half) > cap_mb * 1048576ull) return nullptr;
+    if (need * sizeof(__nv_bfloat16) > cap_mb * 1048576ull) return nullptr;
     if (need > H->wts_cap) {
         if (H->d_wts) cudaFree(H->d_wts);
         H->d_wts = nullptr; H->wts_cap = 0;
-        if (cudaMalloc(&H->d_wts, need * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        if (cudaMalloc(&H->d_wts, need * sizeof(__nv_bfloat16)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
         H->wts_cap = need;
     }
     return H->d_wts;
@@ -517,7 +514,7 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
     int which = 0;
     const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
     if (!sh) return TNLM_INVALID_ARG;
-    __half *wts = (m2 > 1) ? weight_cache(H, *sh, n_slices) : nullptr;   // weights are those of g for all sweeps (L162)
+    __nv_bfloat16 *wts = (m2 > 1) ? weight_cache(H, *sh, n_slices) : nullptr;   // weights are those of g for all sweeps (L162)
     for (int m = 0; m < m2; ++m) {
         const bool last = (m + 1 == m2);
         float *dst;
