@@ -6,7 +6,9 @@
 Metric (BASELINE.json): TNLM Gauss-Jacobi pixel-updates/s (px x phase x iter).  Workload at
 N=1: BASELINE.json configs[1] ("TNLM step alone": 256x256 fp32 x 10 cyclic phases, window 11,
 patch 5, h=0.008, mu=0.1, 10 Gauss-Jacobi sweeps, seed 1).  One step = one
-tnlm_regularize_step call (weights + 10 sweeps + clip) on one slice per GPU.  With N>1 every
+tnlm_regularize_step call (weights + 10 sweeps + clip) on one slice per GPU: 1 launch of
+gj_sweep_kernel<.,.,true> (weights of g, sweep 1, stores the weights as bf16) and 9 launches of
+gj_apply_kernel (sweeps 2..10 from the stored weights, HBM bound).  With N>1 every
 rank runs its own slice (slices are independent: no collective on the data path; weak scaling).
 
 Timed region: K steps, each bracketed by CUDA events on the launching stream; L2 is flushed
@@ -47,9 +49,15 @@ def measured_peaks():
 
 
 def flops_per_px_update(window, patch):
-    """Algorithmic flops of one Gauss-Jacobi pixel update in the separable box-sum form
-    (DESIGN.md "Roofline"): 2 neighbours x W^2 offsets x (2d+4) flops."""
+    """Algorithmic flops of one Gauss-Jacobi pixel update with the weights computed on the fly, in the
+    separable box-sum form: 2 neighbours x W^2 offsets x (2d+4) flops."""
     return 2 * window * window * (2 * patch + 4)
+
+
+def bytes_per_px_update_stored(window):
+    """Algorithmic HBM bytes of one Gauss-Jacobi pixel update from stored weights:
+    2 neighbours x W^2 bf16 weights + g, u read and u' written once (3 x 4 bytes)."""
+    return 2 * window * window * 2 + 12
 
 
 class ClockSampler:
@@ -206,6 +214,17 @@ def run_ours(args):
         barrier()
     launches = h.launch_count - n0
     ms = sum(a.elapsed_time(b) for a, b in ev)
+
+    # ---- per-kernel durations: the same K steps again with the library's event pair around every
+    # launch (CUDA events on the launching stream; kept out of the headline region above)
+    tn.profile_sweeps(h, True)
+    kern = {}
+    for _ in range(args.steps):
+        flush.fill_(1); step()
+        for kind, kms in tn.sweep_times(h):
+            kern.setdefault(kind, []).append(kms)
+    tn.profile_sweeps(h, False)
+    torch.cuda.synchronize()
     t = torch.tensor([ms], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -238,22 +257,45 @@ def run_ours(args):
 
     peaks, peak_src = measured_peaks()
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    hbm_gbs = float(peaks.get("hbm_gbs", 6650.0))
     peak_tf = N_SM * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
-    sweep_s = ms_per_step * 1e-3 / cfg.m2
-    flops_sweep = flops_per_px_update(cfg.window, cfg.patch) * g_np.size
-    achieved_tf = flops_sweep / sweep_s / 1e12
-    roofline = {"kernel": "gj_sweep_kernel (one Gauss-Jacobi sweep: weights + update)", "bound": "alu",
-                "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-                "traffic": None, "us_per_launch": sweep_s * 1e6,
-                "peak_source": f"derived: {N_SM} SM x {FP32_LANES_PER_SM} fp32 lanes x 2 flop x "
-                               f"{sm_mhz:.0f} MHz ({peak_src} sm_max_mhz); no measured FP32 peak exists",
-                "algorithmic_flops_per_px_update": flops_per_px_update(cfg.window, cfg.patch)}
+    n_px = g_np.size
+    traffic = {}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
         try:
-            roofline["traffic"] = json.load(open(traffic_file)).get("gj_sweep_cfg2_dram_bytes_per_launch")
+            traffic = json.load(open(traffic_file))
         except Exception:
-            pass
+            traffic = {}
+    kernels = []
+    step_us = ms_per_step * 1e3
+    for kind, vals in sorted(kern.items()):
+        us = 1e3 * float(np.mean(vals))
+        per_step = len(vals) / args.steps
+        k = {"kernel": {"sweep": "gj_sweep_kernel<PB,RB,false> (weights on the fly + sweep)",
+                        "sweep_store": "gj_sweep_kernel<PB,RB,true> (weights on the fly + sweep, stores bf16 weights)",
+                        "apply": "gj_apply_kernel (sweep from stored bf16 weights)"}[kind],
+             "launches_per_step": per_step, "us_per_launch": us, "share_of_step": per_step * us / step_us}
+        if kind == "apply":
+            gbs = bytes_per_px_update_stored(cfg.window) * n_px / (us * 1e-6) / 1e9
+            k.update({"bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs,
+                      "traffic": traffic.get("gj_apply_cfg2_dram_bytes_per_launch"),
+                      "algorithmic_bytes_per_px_update": bytes_per_px_update_stored(cfg.window)})
+        else:
+            tf = flops_per_px_update(cfg.window, cfg.patch) * n_px / (us * 1e-6) / 1e12
+            k.update({"bound": "alu", "achieved": tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": tf / peak_tf,
+                      "traffic": traffic.get("gj_%s_cfg2_dram_bytes_per_launch" % kind),
+                      "algorithmic_flops_per_px_update": flops_per_px_update(cfg.window, cfg.patch)})
+        kernels.append(k)
+    dominant = max(kernels, key=lambda k: k["share_of_step"]) if kernels else {}
+    roofline = {key: dominant.get(key) for key in ("kernel", "bound", "achieved", "peak", "unit", "frac", "traffic",
+                                                   "us_per_launch", "launches_per_step", "share_of_step")}
+    roofline["peak_source"] = (
+        f"{peak_src} MEASURED_PEAKS.json hbm_gbs (burst copy figure)" if dominant.get("bound") == "hbm" else
+        f"derived: {N_SM} SM x {FP32_LANES_PER_SM} fp32 lanes x 2 flop x {sm_mhz:.0f} MHz ({peak_src} sm_max_mhz); "
+        "no measured FP32 peak exists")
+    roofline["kernels"] = kernels
+    roofline["fp32_peak_tflops_derived"] = peak_tf
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,

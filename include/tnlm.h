@@ -123,6 +123,20 @@ int tnlm_reconstruct_host(tnlm_handle *handle, const float *y_host, const float 
  * next call on the handle.  NULL handle -> message of the last failed tnlm_create. */
 const char *tnlm_last_error(const tnlm_handle *handle);
 
+/* Per-launch device timing of the TNLM kernels (steps 3-5), for benchmarks and rooflines.
+ * tnlm_profile_sweeps(handle, 1) makes every later tnlm_regularize_step / tnlm_reconstruct call
+ * bracket each sweep kernel with a CUDA event pair on the call's stream (0 switches it off;
+ * either call forgets the launches recorded so far).  tnlm_sweep_times waits for the recorded
+ * launches, writes up to `capacity` durations (milliseconds, launch order) into the HOST arrays
+ * ms[] and kind[] (a tnlm_kernel_kind), stores the number recorded in *count, and forgets them. */
+typedef enum {
+    TNLM_KERNEL_SWEEP = 0,       /* weights computed on the fly + one Gauss-Jacobi sweep (Eq. 3/8, Eq. 7) */
+    TNLM_KERNEL_SWEEP_STORE = 1, /* the same, also storing the weights of g^(k) for sweeps 2..m2 */
+    TNLM_KERNEL_APPLY = 2        /* one Gauss-Jacobi sweep of Eq. (7) from the stored weights */
+} tnlm_kernel_kind;
+int tnlm_profile_sweeps(tnlm_handle *handle, int enable);
+int tnlm_sweep_times(tnlm_handle *handle, float *ms, int *kind, int capacity, int *count);
+
 /* Number of CUDA kernels this handle has launched so far (for benchmark bookkeeping). */
 long long tnlm_launch_count(const tnlm_handle *handle);
 

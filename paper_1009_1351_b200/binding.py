@@ -13,7 +13,10 @@ STATUS = {0: "TNLM_OK", 1: "TNLM_INVALID_ARG", 2: "TNLM_CUDA_ERROR", 3: "TNLM_AL
 # every symbol include/tnlm.h declares
 EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "tnlm_cgls_step",
            "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
-           "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version"]
+           "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version",
+           "tnlm_profile_sweeps", "tnlm_sweep_times"]
+
+KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply"}
 
 
 class TnlmError(RuntimeError):
@@ -70,6 +73,8 @@ def library():
         L.tnlm_launch_count.argtypes = [P]
         L.tnlm_launch_count.restype = C.c_longlong
         L.tnlm_version.restype = C.c_char_p
+        L.tnlm_profile_sweeps.argtypes = [P, I]
+        L.tnlm_sweep_times.argtypes = [P, C.POINTER(C.c_float), C.POINTER(I), I, C.POINTER(I)]
         _LIB = L
     return _LIB
 
@@ -175,6 +180,19 @@ def reconstruct(h: Handle, y, w, f0, k_outer, m1, m2, f_out, stream=None):
     h.check(library().tnlm_reconstruct(h.ptr, _dev(y, "y"), _dev(w, "w"), _dev(f0, "f0"), k_outer, m1, m2,
                                        _dev(f_out, "f_out"), S, _stream(stream)))
     return f_out
+
+
+def profile_sweeps(h: Handle, enable: bool):
+    h.check(library().tnlm_profile_sweeps(h.ptr, int(bool(enable))))
+
+
+def sweep_times(h: Handle, capacity: int = 4096):
+    """[(kind name, milliseconds)] of the TNLM kernel launches recorded since the last call."""
+    ms = (C.c_float * capacity)()
+    kind = (C.c_int * capacity)()
+    n = C.c_int(0)
+    h.check(library().tnlm_sweep_times(h.ptr, ms, kind, capacity, C.byref(n)))
+    return [(KERNEL_KINDS.get(kind[i], str(kind[i])), float(ms[i])) for i in range(min(n.value, capacity))]
 
 
 # ---- host-pointer calls: CPU tensors (pinned or pageable); copies happen inside the library ----

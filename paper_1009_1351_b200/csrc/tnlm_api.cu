@@ -52,6 +52,10 @@ struct tnlm_handle {
     double *d_scal = nullptr;
     int scal_cap = 0;
     long long launches = 0;
+    // optional per-launch timing of the TNLM kernels (tnlm_profile_sweeps)
+    bool prof = false;
+    std::vector<cudaEvent_t> prof_ev;     // 2 events per timed launch
+    std::vector<int> prof_kind;
     std::string err;
 };
 
@@ -288,6 +292,7 @@ static void free_ws(tnlm_handle *H)
 extern "C" int tnlm_destroy(tnlm_handle *H)
 {
     if (!H) return TNLM_INVALID_ARG;
+    for (cudaEvent_t e : H->prof_ev) cudaEventDestroy(e);
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
     if (H->d_wts) cudaFree(H->d_wts);
@@ -496,6 +501,49 @@ static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_s
     return H->d_wts;
 }
 
+// Event pair around one kernel launch, on the launching stream.
+static int prof_mark(tnlm_handle *H, int kind, bool begin, cudaStream_t st)
+{
+    if (begin) {
+        const size_t need = 2 * H->prof_kind.size() + 2;
+        while (H->prof_ev.size() < need) {
+            cudaEvent_t e;
+            CU(H, cudaEventCreate(&e));
+            H->prof_ev.push_back(e);
+        }
+        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size()], st));
+        H->prof_kind.push_back(kind);
+    } else {
+        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size() - 1], st));
+    }
+    return TNLM_OK;
+}
+
+extern "C" int tnlm_profile_sweeps(tnlm_handle *H, int enable)
+{
+    if (!H) return TNLM_INVALID_ARG;
+    H->err.clear();
+    H->prof = enable != 0;
+    H->prof_kind.clear();
+    return TNLM_OK;
+}
+
+extern "C" int tnlm_sweep_times(tnlm_handle *H, float *ms, int *kind, int capacity, int *count)
+{
+    if (!H) return TNLM_INVALID_ARG;
+    H->err.clear();
+    if (!count || capacity < 0 || (capacity > 0 && (!ms || !kind))) return fail(H, TNLM_INVALID_ARG, "count, and ms/kind when capacity > 0, must not be NULL");
+    const int n = (int)H->prof_kind.size();
+    *count = n;
+    for (int i = 0; i < n && i < capacity; ++i) {
+        CU(H, cudaEventSynchronize(H->prof_ev[2 * i + 1]));
+        CU(H, cudaEventElapsedTime(&ms[i], H->prof_ev[2 * i], H->prof_ev[2 * i + 1]));
+        kind[i] = H->prof_kind[i];
+    }
+    H->prof_kind.clear();
+    return TNLM_OK;
+}
+
 // g -> f_out; g and f_out are distinct device buffers or the same buffer.
 static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_out, int n_slices, cudaStream_t st)
 {
@@ -520,9 +568,13 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
         float *dst;
         if (last && !alias) dst = f_out;
         else { dst = pp[which]; if (dst == src) { which ^= 1; dst = pp[which]; } }
-        if (m == 0 || !wts) rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
+        const bool computes = (m == 0 || !wts);
+        const int kind = computes ? (wts ? TNLM_KERNEL_SWEEP_STORE : TNLM_KERNEL_SWEEP) : TNLM_KERNEL_APPLY;
+        if (H->prof && (rc = prof_mark(H, kind, true, st))) return rc;
+        if (computes) rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
         else rc = launch_apply(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
         if (rc) return rc;
+        if (H->prof && (rc = prof_mark(H, kind, false, st))) return rc;
         src = dst;
         which ^= 1;
     }
