@@ -10,14 +10,15 @@ namespace tnlm {
 // expressions on it (ray_cell below), so P^T is the exact transpose of P entry by entry.
 //   steep ray (|dy| >= |dx|): column coordinate xi(eta) = p0 + m*eta   (grid units, pixel c = [c,c+1))
 //   shallow ray             : row    coordinate eta(xi) = p0 + m*xi
-//   len  = length of the ray inside one full row (steep) / column (shallow), in mm
-//   inva = 1/|m| (0 if m == 0)
-//   flag : bit0 = steep; lo/hi = inclusive range of rows (steep) / columns (shallow) to walk
+//   plo  = p0 + min(m, 0): the smaller of the two coordinates at which the ray enters / leaves
+//          row (column) q is lo(q) = m*q + plo; the larger one is lo + |m| <= lo + 1
+//   len  = length of the ray inside one full row (steep, stored > 0) / column (shallow, stored < 0), mm
+//   inva = 1/|m| (1e30 if m == 0)
 struct __align__(16) RayEntry {
-    float p0, m, len, inva;
+    float plo, m, len, inva;
 };
 struct __align__(8) RayRange {
-    short lo, hi;      // empty if hi < lo
+    short lo, hi;      // inclusive range of rows (steep) / columns (shallow) to walk; empty if hi < lo
     int steep;
 };
 
@@ -26,27 +27,30 @@ struct Geom {
     float pix;                 // mm
     float sdd_over_pitch;      // bins per radian of fan angle
     float bin_centre;          // (B-1)/2 - bin_offset
-    float half_diag;           // pix/sqrt(2) mm
+    float hw_scale;            // 1.02 * (pix/sqrt(2)) * sdd_over_pitch: half-width of a pixel in bins x distance
 };
 
-// One row (steep) or column (shallow) of one ray: the at most two cells it touches there and
-// the lengths inside them.  q = row index (steep) / column index (shallow).
-// Returns c0,c1 (cell indices along the other axis; c1 >= c0) and w0,w1 (mm).  When the ray
-// stays in one cell, c1 == c0 and w1 == 0.  Explicit intrinsics: no contraction differences
-// between the two kernels that inline this.
-__device__ __forceinline__ void ray_cell(const RayEntry e, int q, int &c0, int &c1, float &w0, float &w1)
+// floor() of |x| < 2^22 without the conversion unit: round-down add of 1.5*2^23 leaves floor(x)
+// in the low mantissa bits (FADD.RM on the FP32 pipe; FRND/F2I would go to the 16-lane XU pipe).
+constexpr float FLOOR_MAGIC = 12582912.0f;
+constexpr int FLOOR_MAGIC_BITS = 0x4B400000;
+
+// One row (steep) or column (shallow) of one ray: the at most two cells it touches there and the
+// lengths inside them.  qf = row index (steep) / column index (shallow) as a float.  Returns c0 (the
+// cell holding the smaller coordinate; the other cell, if any, is c0+1) and w0, w1 (mm); w1 == 0
+// when the ray stays in one cell.  The split is at the cell boundary b = c0+1: the fraction of the
+// crossing below b is sat((b - lo)/|m|), which is 1 when the ray does not reach b.  Explicit
+// intrinsics: no contraction differences between the two kernels that inline this.
+__device__ __forceinline__ void ray_cell(const float plo, const float m, const float alen, const float inva,
+                                         const float qf, int &c0, float &w0, float &w1)
 {
-    const float fq = (float)q;
-    const float xa = __fmaf_rn(e.m, fq, e.p0);
-    const float xb = __fmaf_rn(e.m, fq + 1.0f, e.p0);
-    const float lo = fminf(xa, xb), hi = fmaxf(xa, xb);
-    const float f0 = floorf(lo), f1 = floorf(hi);
-    c0 = (int)f0;
-    c1 = (int)f1;
-    float frac = 1.0f;
-    if (f1 > f0) frac = __saturatef(__fmul_rn(__fsub_rn(f1, lo), e.inva));
-    w0 = __fmul_rn(e.len, frac);
-    w1 = __fsub_rn(e.len, w0);
+    const float lo = __fmaf_rn(m, qf, plo);
+    const float f0r = __fadd_rd(lo, FLOOR_MAGIC);
+    c0 = __float_as_int(f0r) - FLOOR_MAGIC_BITS;
+    const float t = __fsub_rn(__fsub_rn(f0r, FLOOR_MAGIC), lo);       // floor(lo) - lo in (-1, 0]
+    const float frac = __saturatef(__fmaf_rn(t, inva, inva));          // ((c0+1) - lo)/|m|, clamped
+    w0 = __fmul_rn(alen, frac);
+    w1 = __fsub_rn(alen, w0);
 }
 
 __device__ __forceinline__ float warp_sum(float v)

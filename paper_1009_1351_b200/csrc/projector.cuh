@@ -13,13 +13,54 @@ enum FwdMode {
     FWD_SCALE = 2   // out0 = sw*(P img) = q ; red += ||q||^2             (CGLS step 1, L112)
 };
 
+// atan on the fan-angle range: odd minimax polynomial on [-1, 1] (Abramowitz & Stegun 4.4.49,
+// |error| <= 2e-8 rad, i.e. < 1e-4 bin), atanf beyond 45 degrees.  Only the conservative candidate
+// range of the backprojector depends on it; membership and lengths come from ray_cell.
+__device__ __forceinline__ float fan_angle(float t)
+{
+    if (fabsf(t) > 1.0f) return atanf(t);
+    const float z = t * t;
+    float p = 0.0028662257f;
+    p = fmaf(p, z, -0.0161657367f);
+    p = fmaf(p, z, 0.0429096138f);
+    p = fmaf(p, z, -0.0752896400f);
+    p = fmaf(p, z, 0.1065626393f);
+    p = fmaf(p, z, -0.1420889944f);
+    p = fmaf(p, z, 0.1999355085f);
+    p = fmaf(p, z, -0.3333314528f);
+    return fmaf(p * z, t, t);
+}
+
 // ------------------------------------------------------------------------------ forward
 // grid = (ceil(V*B/256), S*N); block = 256.  Adjacent threads = adjacent bins of a view, so a
 // warp walks neighbouring pixels of the same image rows (coalesced, L1-resident gathers).
+// imgT[prob][c][r] = img[prob][r][c]: shallow rays walk columns, and 32 neighbouring bins of a warp
+// sit in ~18 different image rows there (18 cache lines per load); in the transposed copy they are
+// neighbours again.  grid = (ceil(nx/32), ceil(ny/32), S*N), block = (32, 8).
+__global__ void __launch_bounds__(256)
+transpose_kernel(const float *__restrict__ img, float *__restrict__ imgT, int nx, int ny)
+{
+    __shared__ float tile[32][33];
+    const size_t base = (size_t)blockIdx.z * nx * ny;
+    const int c = blockIdx.x * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int r = blockIdx.y * 32 + threadIdx.y + j;
+        tile[threadIdx.y + j][threadIdx.x] = (r < ny && c < nx) ? __ldg(img + base + (size_t)r * nx + c) : 0.f;
+    }
+    __syncthreads();
+    const int rT = blockIdx.y * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int cT = blockIdx.x * 32 + threadIdx.y + j;
+        if (rT < ny && cT < nx) imgT[base + (size_t)cT * ny + rT] = tile[threadIdx.x][threadIdx.y + j];
+    }
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(256)
 project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
-               const float *__restrict__ img, const float *__restrict__ y,
+               const float *__restrict__ img, const float *__restrict__ imgT, const float *__restrict__ y,
                const float *__restrict__ w, float *__restrict__ out0, float *__restrict__ out1,
                double *__restrict__ red)
 {
@@ -32,23 +73,28 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
         const RayEntry e = tab[(size_t)phase * nray + ray];
         const RayRange rg = rng[(size_t)phase * nray + ray];
         const float *__restrict__ im = img + (size_t)prob * G.nx * G.ny;
+        const float alen = fabsf(e.len);
         float acc0 = 0.f, acc1 = 0.f;
+        float qf = (float)rg.lo;
         if (rg.steep) {
             const int nx = G.nx;
-            for (int q = rg.lo; q <= rg.hi; ++q) {
-                int c0, c1; float w0, w1;
-                ray_cell(e, q, c0, c1, w0, w1);
-                const float *row = im + (size_t)q * nx;
+            const float *__restrict__ row = im + (size_t)rg.lo * nx;
+#pragma unroll 4
+            for (int q = rg.lo; q <= rg.hi; ++q, qf += 1.0f, row += nx) {
+                int c0; float w0, w1;
+                ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
                 if ((unsigned)c0 < (unsigned)nx) acc0 = fmaf(w0, __ldg(row + c0), acc0);
-                if (c1 != c0 && (unsigned)c1 < (unsigned)nx) acc1 = fmaf(w1, __ldg(row + c1), acc1);
+                if ((unsigned)(c0 + 1) < (unsigned)nx) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
             }
-        } else {
-            const int nx = G.nx, ny = G.ny;
-            for (int q = rg.lo; q <= rg.hi; ++q) {
-                int c0, c1; float w0, w1;
-                ray_cell(e, q, c0, c1, w0, w1);
-                if ((unsigned)c0 < (unsigned)ny) acc0 = fmaf(w0, __ldg(im + (size_t)c0 * nx + q), acc0);
-                if (c1 != c0 && (unsigned)c1 < (unsigned)ny) acc1 = fmaf(w1, __ldg(im + (size_t)c1 * nx + q), acc1);
+        } else {                                   // shallow: the same walk over the rows of the transposed image
+            const int ny = G.ny;
+            const float *__restrict__ row = imgT + (size_t)prob * G.nx * ny + (size_t)rg.lo * ny;
+#pragma unroll 4
+            for (int q = rg.lo; q <= rg.hi; ++q, qf += 1.0f, row += ny) {
+                int c0; float w0, w1;
+                ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
+                if ((unsigned)c0 < (unsigned)ny) acc0 = fmaf(w0, __ldg(row + c0), acc0);
+                if ((unsigned)(c0 + 1) < (unsigned)ny) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
             }
         }
         const float p = acc0 + acc1;
@@ -103,31 +149,29 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__r
     if (inside) {
         const float X = ((float)c - 0.5f * (float)(G.nx - 1)) * G.pix;
         const float Y = ((float)r - 0.5f * (float)(G.ny - 1)) * G.pix;
+        const float rf = (float)r, cf = (float)c;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
-        const RayEntry *__restrict__ tb = tab + (size_t)phase * V * B;
-        const RayRange *__restrict__ rb = rng + (size_t)phase * V * B;
+        const float4 *__restrict__ tb = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg = sino + (size_t)prob * V * B;
-        for (int v = 0; v < V; ++v) {
+        for (int v = 0; v < V; ++v, tb += B, sg += B) {
             const float4 vw = __ldg(vt + v);                 // sx, sy, cos th, sin th
             const float px = X - vw.x, py = Y - vw.y;
             const float dot = -(vw.z * px + vw.w * py);      // along the central ray (> 0)
             const float crs = vw.w * px - vw.z * py;         // ccw from the central ray
-            const float gam = atanf(__fdividef(crs, dot));
-            const float kc = fmaf(gam, G.sdd_over_pitch, G.bin_centre);
-            const float hw = fmaf(G.half_diag * rsqrtf(px * px + py * py), G.sdd_over_pitch * 1.02f, 0.05f);
-            const int k_lo = max(0, (int)ceilf(kc - hw));
-            const int k_hi = min(B - 1, (int)floorf(kc + hw));
+            const float rdot = __fdividef(1.0f, dot);
+            const float kc = fmaf(fan_angle(crs * rdot), G.sdd_over_pitch, G.bin_centre);
+            // the pixel's angular half-width is <= (pix/sqrt 2)/distance <= (pix/sqrt 2)/dot
+            const float hw = fmaf(G.hw_scale, rdot, 0.05f);
+            const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
+            const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             for (int k = k_lo; k <= k_hi; ++k) {
-                const float4 e4 = __ldg(reinterpret_cast<const float4 *>(tb + (size_t)v * B + k));
-                RayEntry e; e.p0 = e4.x; e.m = e4.y; e.len = e4.z; e.inva = e4.w;
-                const int steep = __ldg(&rb[(size_t)v * B + k].steep);
-                int c0, c1; float w0, w1;
-                ray_cell(e, steep ? r : c, c0, c1, w0, w1);
+                const float4 e4 = __ldg(tb + k);             // plo, m, len (sign = steep), inva
+                const bool steep = e4.z > 0.f;
+                int c0; float w0, w1;
+                ray_cell(e4.x, e4.y, fabsf(e4.z), e4.w, steep ? rf : cf, c0, w0, w1);
                 const int me = steep ? c : r;
-                float wgt = 0.f;
-                if (c0 == me) wgt = w0;
-                else if (c1 == me) wgt = w1;
-                acc = fmaf(wgt, __ldg(sg + (size_t)v * B + k), acc);
+                const float wgt = (c0 == me) ? w0 : ((c0 + 1 == me) ? w1 : 0.f);
+                acc = fmaf(wgt, __ldg(sg + k), acc);
             }
         }
         out[(size_t)prob * G.nx * G.ny + (size_t)r * G.nx + c] = acc;

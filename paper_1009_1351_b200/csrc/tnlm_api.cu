@@ -44,6 +44,7 @@ struct tnlm_handle {
     int ws_slices = 0;
     float *d_s = nullptr, *d_t = nullptr, *d_g = nullptr, *d_f = nullptr;  // images
     float *d_ua = nullptr, *d_ub = nullptr;                                  // sweep ping-pong
+    float *d_imT = nullptr;                                                  // transposed image of the forward projector
     float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr;                   // sinograms
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
     __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
@@ -113,8 +114,10 @@ static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, st
                 const double p0 = steep ? xs - m * es : es - m * xs;
                 const double len = g.pixel_mm / (steep ? std::fabs(dy) : std::fabs(dx));
                 RayEntry e;
-                e.p0 = (float)p0; e.m = (float)m; e.len = (float)len;
-                e.inva = (e.m != 0.f) ? 1.0f / std::fabs(e.m) : 0.f;
+                e.m = (float)m;
+                e.plo = (float)(p0 + std::fmin((double)e.m, 0.0));
+                e.len = (float)(steep ? len : -len);
+                e.inva = (e.m != 0.f) ? 1.0f / std::fabs(e.m) : 1e30f;
                 // walk range along the major axis: where the minor coordinate is within [-1, n+1]
                 const int n_major = steep ? ny : nx, n_minor = steep ? nx : ny;
                 int lo = 0, hi = n_major - 1;
@@ -262,7 +265,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         G.pix = (float)g.pixel_mm;
         G.sdd_over_pitch = (float)(g.sdd_mm / g.bin_pitch_mm);
         G.bin_centre = (float)(0.5 * (g.n_bins - 1) - g.bin_offset);
-        G.half_diag = (float)(g.pixel_mm * 0.70710678118654752);
+        G.hw_scale = (float)(1.02 * g.pixel_mm * 0.70710678118654752 * g.sdd_mm / g.bin_pitch_mm);
         std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views;
         build_tables(g, nx, ny, n_phase, tab, rng, views);
         bool ok = cudaMalloc(&H->d_tab, tab.size() * sizeof(RayEntry)) == cudaSuccess &&
@@ -284,7 +287,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
 
 static void free_ws(tnlm_handle *H)
 {
-    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_r, &H->d_rw, &H->d_q, &H->d_yh, &H->d_wh};
+    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_r, &H->d_rw, &H->d_q, &H->d_yh, &H->d_wh};
     for (float **b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     H->ws_slices = 0;
 }
@@ -337,8 +340,13 @@ static int launch_project(tnlm_handle *H, const float *img, const float *y, cons
                           float *out1, double *red, int n_slices, cudaStream_t st)
 {
     const int nray = H->G.n_views * H->G.n_bins;
+    int rc = need(H, &H->d_imT, img_count(H));
+    if (rc) return rc;
+    dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, n_slices * H->n_phase);
+    transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(img, H->d_imT, H->nx, H->ny);
+    LAUNCHED(H);
     dim3 grid((nray + 255) / 256, n_slices * H->n_phase);
-    project_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, y, w, out0, out1, red);
+    project_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, H->d_imT, y, w, out0, out1, red);
     LAUNCHED(H);
     return TNLM_OK;
 }
@@ -355,6 +363,7 @@ extern "C" int tnlm_project(tnlm_handle *H, const float *img, float *sino, int n
     int rc = check_common(H, n_slices, true);
     if (rc) return rc;
     if (!img || !sino) return fail(H, TNLM_INVALID_ARG, "img and sino must not be NULL");
+    if ((rc = ensure_ws(H, n_slices))) return rc;
     return launch_project<FWD_PLAIN>(H, img, nullptr, nullptr, sino, nullptr, nullptr, n_slices, (cudaStream_t)stream);
 }
 
