@@ -41,16 +41,23 @@ constexpr int FLOOR_MAGIC_BITS = 0x4B400000;
 // when the ray stays in one cell.  The split is at the cell boundary b = c0+1: the fraction of the
 // crossing below b is sat((b - lo)/|m|), which is 1 when the ray does not reach b.  Explicit
 // intrinsics: no contraction differences between the two kernels that inline this.
-__device__ __forceinline__ void ray_cell(const float plo, const float m, const float alen, const float inva,
-                                         const float qf, int &c0, float &w0, float &w1)
+__device__ __forceinline__ void ray_cell_f(const float plo, const float m, const float alen, const float inva,
+                                           const float qf, float &f0r, float &f0, float &w0, float &w1)
 {
     const float lo = __fmaf_rn(m, qf, plo);
-    const float f0r = __fadd_rd(lo, FLOOR_MAGIC);
-    c0 = __float_as_int(f0r) - FLOOR_MAGIC_BITS;
-    const float t = __fsub_rn(__fsub_rn(f0r, FLOOR_MAGIC), lo);       // floor(lo) - lo in (-1, 0]
+    f0r = __fadd_rd(lo, FLOOR_MAGIC);                                  // bits: FLOOR_MAGIC_BITS + floor(lo)
+    f0 = __fsub_rn(f0r, FLOOR_MAGIC);                                  // floor(lo) as a float, exactly
+    const float t = __fsub_rn(f0, lo);                                 // floor(lo) - lo in (-1, 0]
     const float frac = __saturatef(__fmaf_rn(t, inva, inva));          // ((c0+1) - lo)/|m|, clamped
     w0 = __fmul_rn(alen, frac);
     w1 = __fsub_rn(alen, w0);
+}
+__device__ __forceinline__ void ray_cell(const float plo, const float m, const float alen, const float inva,
+                                         const float qf, int &c0, float &w0, float &w1)
+{
+    float f0r, f0;
+    ray_cell_f(plo, m, alen, inva, qf, f0r, f0, w0, w1);
+    c0 = __float_as_int(f0r) - FLOOR_MAGIC_BITS;
 }
 
 __device__ __forceinline__ float warp_sum(float v)

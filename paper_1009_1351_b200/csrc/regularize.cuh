@@ -75,6 +75,7 @@ struct SweepParams {
     float margin;           // the delta = 0 weight is 2^-margin (90)
     float z_limit;          // a side whose weight sum is not below this is recomputed exactly
     int clip;               // apply max(.,0) to the output
+    int ap_ns;              // gj_apply_kernel: stages of its bulk-copy ring
 };
 
 // Shared-memory tile geometry (words), shared by host (sizing) and device.
@@ -468,14 +469,14 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
 // over, nothing else synchronises.  u_j of both neighbours is staged with its halo in shared
 // memory, zero-filled outside the image (excluded candidates carry weight 0 in the chunks).
 // grid.x = (S*N) * ceil(ny / rb) * tiles_x; block = 32 * (rb + 1).
-constexpr int AP_SO = 4;     // offsets (consecutive dc of one dr) per stage
-constexpr int AP_NS = 4;     // stages in flight
+constexpr int AP_SO = 4;         // offsets (consecutive dc of one dr) per stage
+constexpr int AP_NS_MAX = 8;     // stages in flight: p.ap_ns, chosen per launch (wave quantisation vs bytes in flight)
 __host__ __device__ inline int apply_uw(int window) { return 124 + 4 * ((window + 3) / 4 + 1); }
-__host__ __device__ inline size_t apply_smem_bytes(int window, int rb)
+__host__ __device__ inline size_t apply_smem_bytes(int window, int rb, int ns)
 {
     const int a = (window - 1) / 2;
-    return (size_t)AP_NS * AP_SO * rb * SW_TW * sizeof(__nv_bfloat16) + (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) +
-           2 * AP_NS * sizeof(uint64_t);
+    return (size_t)ns * AP_SO * rb * SW_TW * sizeof(__nv_bfloat16) + (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) +
+           2 * AP_NS_MAX * sizeof(uint64_t);
 }
 
 __global__ void __launch_bounds__(352)
@@ -489,10 +490,11 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     const int rb = p.rb, urows = rb + 2 * a;
     const size_t wstride = (size_t)rb * SW_TW;      // halves per offset
     extern __shared__ float4 smem4[];
-    __nv_bfloat16 *sW = reinterpret_cast<__nv_bfloat16 *>(smem4);                                 // [AP_NS][AP_SO][rb][128]
+    const int AP_NS = p.ap_ns;
+    __nv_bfloat16 *sW = reinterpret_cast<__nv_bfloat16 *>(smem4);                   // [AP_NS][AP_SO][rb][128]
     float *sU = reinterpret_cast<float *>(sW + (size_t)AP_NS * AP_SO * wstride);    // [2][urows][UW]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sU + 2 * urows * UW);             // [AP_NS], then empty[AP_NS]
-    uint64_t *empty = full + AP_NS;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sU + 2 * urows * UW);             // [AP_NS_MAX], then empty[AP_NS_MAX]
+    uint64_t *empty = full + AP_NS_MAX;
 
     const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
     const int img = blockIdx.x / tiles_per_img;
@@ -504,7 +506,7 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < AP_NS; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, rb); }
+        for (int i = 0; i < p.ap_ns; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, rb); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -517,9 +519,9 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 
     if (warp == rb) {                               // ---- producer warp: one lane issues the bulk copies
         if (lane == 0) {
+            int slot = 0, round = 0;
             for (int t = 0; t < T; ++t) {
-                const int slot = t % AP_NS;
-                if (t >= AP_NS) mbar_wait(empty + slot, ((t / AP_NS) - 1) & 1);
+                if (round > 0) mbar_wait(empty + slot, (round - 1) & 1);
                 const int sd = t / stages_per_side, rem = t - sd * stages_per_side;
                 const int dr = rem / nchunk, k = rem - dr * nchunk;
                 const int noff = min(AP_SO, W - AP_SO * k);
@@ -527,6 +529,7 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                 mbar_expect_tx(full + slot, bytes);
                 bulk_g2s(sW + (size_t)slot * AP_SO * wstride, chunk0 + sd * side_stride + (size_t)(dr * W + AP_SO * k) * wstride,
                          bytes, full + slot);
+                if (++slot == AP_NS) { slot = 0; ++round; }
             }
         }
         return;
@@ -543,7 +546,8 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 
     const int r = tile_r0 + warp, c0 = tile_c0 + C * lane;
     float nbsum[C] = {0.f, 0.f, 0.f, 0.f};
-    int t = 0;
+    int slot = 0;
+    unsigned parity = 0;
 #pragma unroll 1
     for (int s = 0; s < 2; ++s) {
         float Z[C] = {0.f, 0.f, 0.f, 0.f}, A[C] = {0.f, 0.f, 0.f, 0.f};
@@ -551,18 +555,18 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
         for (int dr = 0; dr < W; ++dr) {
             const float4 *__restrict__ up = reinterpret_cast<const float4 *>(sU + (s * urows + warp + dr) * UW) + lane;
 #pragma unroll 1
-            for (int k = 0; k < nchunk; ++k, ++t) {
-                const int slot = t % AP_NS;
+            for (int k = 0; k < nchunk; ++k) {
                 const float4 u0 = up[k], u1 = up[k + 1];
                 const float uw[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
                 const int noff = min(AP_SO, W - AP_SO * k);
-                mbar_wait(full + slot, (t / AP_NS) & 1);
+                mbar_wait(full + slot, parity);
                 const uint2 *__restrict__ wq = reinterpret_cast<const uint2 *>(sW + (size_t)slot * AP_SO * wstride + warp * SW_TW) + lane;
                 uint2 wv[AP_SO];
 #pragma unroll
                 for (int jj = 0; jj < AP_SO; ++jj) wv[jj] = wq[(jj < noff ? jj : 0) * (wstride / 4)];
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + slot);           // values are in registers: slot is free
+                if (++slot == AP_NS) { slot = 0; parity ^= 1u; }
 #pragma unroll
                 for (int jj = 0; jj < AP_SO; ++jj) {
                     if (jj < noff) {

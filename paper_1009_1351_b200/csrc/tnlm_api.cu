@@ -36,6 +36,7 @@ struct tnlm_handle {
     SweepParams R{};
     std::vector<SweepShape> shapes;   // launchable sweep shapes for this (window, patch)
     int n_sm = 148;
+    size_t smem_per_sm = 233472;
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
@@ -246,12 +247,13 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     R.z_limit = 1.0e38f;
     R.clip = 0;
     {
-        H->apply_smem = apply_smem_bytes(window, 10);   // rb <= 10
+        H->apply_smem = std::min(apply_smem_bytes(window, 10, AP_NS_MAX), (size_t)prop.sharedMemPerBlockOptin);   // rb <= 10
         ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)H->apply_smem);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
     }
     H->n_sm = prop.multiProcessorCount;
+    H->smem_per_sm = prop.sharedMemPerMultiprocessor;
     ce = build_sweep_shapes(H, (size_t)prop.sharedMemPerBlockOptin);
     if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "sweep kernel setup"); }
     if (H->shapes.empty()) {
@@ -485,7 +487,24 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
-    gj_apply_kernel<<<(unsigned)ctas, 32 * (sh.rb + 1), apply_smem_bytes(H->window, sh.rb), st>>>(R, g, u, out, wts);
+    // ring depth: the most stages whose shared memory still leaves the last wave best filled
+    const int threads = 32 * (sh.rb + 1);
+    double best_eff = -1.0;
+    size_t smem = 0;
+    int want_ns = 0;                                     // tuning override for experiments
+    if (const char *ev = std::getenv("TNLM_APPLY_NS")) want_ns = std::atoi(ev);
+    for (int ns = AP_NS_MAX; ns >= 2; --ns) {
+        if (want_ns && ns != want_ns) continue;
+        const size_t sm = apply_smem_bytes(H->window, sh.rb, ns);
+        if (sm > H->apply_smem) continue;
+        const long long occ = std::min<long long>((long long)(H->smem_per_sm / (sm + 1024)), 2048 / threads);
+        if (occ < 1) continue;
+        const long long cap = occ * H->n_sm, waves = (ctas + cap - 1) / cap;
+        const double eff = (double)ctas / (double)(waves * cap) + 1e-3 * ns;     // ties: deeper ring
+        if (eff > best_eff) { best_eff = eff; R.ap_ns = ns; smem = sm; }
+    }
+    if (best_eff < 0.0) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+    gj_apply_kernel<<<(unsigned)ctas, threads, smem, st>>>(R, g, u, out, wts);
     LAUNCHED(H);
     return TNLM_OK;
 }
