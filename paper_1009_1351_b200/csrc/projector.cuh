@@ -14,11 +14,11 @@ enum FwdMode {
 };
 
 // atan on the fan-angle range: odd minimax polynomial on [-1, 1] (Abramowitz & Stegun 4.4.49,
-// |error| <= 2e-8 rad, i.e. < 1e-4 bin), atanf beyond 45 degrees.  Only the conservative candidate
-// range of the backprojector depends on it; membership and lengths come from ray_cell.
-__device__ __forceinline__ float fan_angle(float t)
+// |error| <= 2e-8 rad, i.e. < 1e-4 bin); detectors wider than +-40 degrees use atanf (kernel
+// template POLY = false).  Only the conservative candidate range of the backprojector depends on
+// it; membership and lengths come from ray_cell.
+__device__ __forceinline__ float fan_angle_poly(float t)
 {
-    if (fabsf(t) > 1.0f) return atanf(t);
     const float z = t * t;
     float p = 0.0028662257f;
     p = fmaf(p, z, -0.0161657367f);
@@ -128,28 +128,32 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
 }
 
 // ----------------------------------------------------------------------------- adjoint
-// grid = (ceil(nx/32), ceil(ny/BP_ROWS), S*N); block = (32, BP_ROWS).  One thread per pixel,
-// loop over the views of its phase; per view the candidate bins are those whose fan angle is
-// within the pixel's angular footprint (conservative superset); each candidate's ray_cell for
-// this pixel's row (steep ray) or column (shallow ray) decides membership and gives the length.
+// grid = (ceil(nx/16), ceil(ny/32), S*N); block = 128 threads.  One thread per 2 x 2 pixel block
+// (rows r0, r0+1, columns c0, c0+1; a warp covers 16 x 8 pixels), loop over the views of its
+// phase.  Per view the candidate bins are those whose fan angle is within the block's angular
+// footprint (conservative superset).  A steep candidate is evaluated in rows r0 and r0+1, a
+// shallow one in columns c0 and c0+1: each ray_cell serves the two block pixels of that row
+// (column), so the block costs 2 evaluations per candidate instead of 4, and the same expressions
+// as the forward projector decide membership and give the lengths (exact transpose).
 // red (optional) += ||out||^2 of this problem.
-#define BP_ROWS 4
-__global__ void __launch_bounds__(32 * BP_ROWS)
-backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
-                   const float4 *__restrict__ views, const float *__restrict__ sino,
-                   float *__restrict__ out, double *__restrict__ red)
+template <bool POLY>
+__global__ void __launch_bounds__(128)
+backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__restrict__ views,
+                   const float *__restrict__ sino, float *__restrict__ out, double *__restrict__ red)
 {
     const int prob = blockIdx.z;
     const int phase = prob % G.n_phase;
-    const int c = blockIdx.x * 32 + threadIdx.x;
-    const int r = blockIdx.y * BP_ROWS + threadIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c0 = blockIdx.x * 16 + 2 * (lane & 7);
+    const int r0 = blockIdx.y * 32 + warp * 8 + 2 * (lane >> 3);
     const int V = G.n_views, B = G.n_bins;
-    const bool inside = (c < G.nx) && (r < G.ny);
-    float acc = 0.f;
+    const bool inside = (c0 < G.nx) && (r0 < G.ny);
+    float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;
     if (inside) {
-        const float X = ((float)c - 0.5f * (float)(G.nx - 1)) * G.pix;
-        const float Y = ((float)r - 0.5f * (float)(G.ny - 1)) * G.pix;
-        const float rf = (float)r, cf = (float)c, dcr = cf - rf;
+        // block centre
+        const float X = ((float)c0 + 0.5f - 0.5f * (float)(G.nx - 1)) * G.pix;
+        const float Y = ((float)r0 + 0.5f - 0.5f * (float)(G.ny - 1)) * G.pix;
+        const float rf = (float)r0, cf = (float)c0, dcr = cf - rf;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
         const float4 *__restrict__ tb = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg = sino + (size_t)prob * V * B;
@@ -158,47 +162,67 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__r
             const float px = X - vw.x, py = Y - vw.y;
             const float dot = -(vw.z * px + vw.w * py);      // along the central ray (> 0)
             const float crs = vw.w * px - vw.z * py;         // ccw from the central ray
-            const float rdot = __fdividef(1.0f, dot);
-            const float kc = fmaf(fan_angle(crs * rdot), G.sdd_over_pitch, G.bin_centre);
-            // the pixel's angular half-width is <= (pix/sqrt 2)/distance <= (pix/sqrt 2)/dot
-            const float hw = fmaf(G.hw_scale, rdot, 0.05f);
+            float rdot;
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rdot) : "f"(dot));
+            const float t = crs * rdot;
+            const float kc = fmaf(POLY ? fan_angle_poly(t) : atanf(t), G.sdd_over_pitch, G.bin_centre);
+            // the block's angular half-width is <= (pix*sqrt 2)/distance <= (pix*sqrt 2)/dot
+            const float hw = fmaf(2.0f * G.hw_scale, rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const float4 *__restrict__ tbk = tb + k_lo;
             const float *__restrict__ sgk = sg + k_lo;
-            // Membership and length of each candidate by FP32-pipe arithmetic only (the integer /
-            // compare pipe is half rate and was the bottleneck at 76 %): s = 1 for a steep ray, 0 for a
-            // shallow one; the ray is tested in this pixel's row (steep) or column (shallow); the pixel
-            // index along the other axis minus floor(lo) is 0 (-> w0), 1 (-> w1) or neither (-> 0).
+            // Membership and lengths by FP32-pipe arithmetic (the integer / compare pipe is half rate
+            // and was the bottleneck): st = 1 for a steep ray, 0 for a shallow one; evaluation j is in
+            // row r0+j (steep) or column c0+j (shallow); with dm = (index of the block's first pixel
+            // along the other axis) - floor(lo): that pixel holds w0 if dm = 0, w1 if dm = 1, and its
+            // neighbour holds w0 if dm = -1, w1 if dm = 0.
             for (int n = k_hi - k_lo; n >= 0; --n, ++tbk, ++sgk) {
                 const float4 e4 = __ldg(tbk);                // plo, m, len (sign = steep), inva
                 const float sv = __ldg(sgk);
                 const float st = __saturatef(e4.z * 1.0e30f);
                 const float qf = __fmaf_rn(st, -dcr, cf);    // rf (steep) or cf (shallow), exactly
                 const float mef = __fmaf_rn(st, dcr, rf);    // cf (steep) or rf (shallow), exactly
-                float f0r, f0, w0, w1;
-                ray_cell_f(e4.x, e4.y, fabsf(e4.z), e4.w, qf, f0r, f0, w0, w1);
-                const float dm = __fsub_rn(mef, f0);         // 0: this pixel holds w0; 1: it holds w1
-                const float i0 = __saturatef(1.0f - fabsf(dm));
-                const float i1 = __saturatef(1.0f - fabsf(dm - 1.0f));
-                const float wgt = __fmaf_rn(w0, i0, __fmul_rn(w1, i1));   // w0, w1 or 0, exactly
-                acc = fmaf(wgt, sv, acc);
+                const float alen = fabsf(e4.z);
+                float wA[2], wB[2];
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    float f0r, f0, w0, w1;
+                    ray_cell_f(e4.x, e4.y, alen, e4.w, qf + (float)j, f0r, f0, w0, w1);
+                    const float dm = __fsub_rn(mef, f0);
+                    const float i0 = __saturatef(1.0f - fabsf(dm));
+                    const float i1 = __saturatef(1.0f - fabsf(dm - 1.0f));
+                    const float im = __saturatef(1.0f - fabsf(dm + 1.0f));
+                    wA[j] = __fmaf_rn(w0, i0, __fmul_rn(w1, i1));     // w0, w1 or 0, exactly
+                    wB[j] = __fmaf_rn(w0, im, __fmul_rn(w1, i0));
+                }
+                const bool steep = e4.z > 0.f;
+                a00 = fmaf(wA[0], sv, a00);
+                a11 = fmaf(wB[1], sv, a11);
+                a01 = fmaf(steep ? wB[0] : wA[1], sv, a01);
+                a10 = fmaf(steep ? wA[1] : wB[0], sv, a10);
             }
         }
-        out[(size_t)prob * G.nx * G.ny + (size_t)r * G.nx + c] = acc;
+        float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + (size_t)r0 * G.nx + c0;
+        const bool c1in = c0 + 1 < G.nx, r1in = r0 + 1 < G.ny;
+        if (c1in && ((G.nx & 1) == 0) && ((reinterpret_cast<uintptr_t>(out) & 7) == 0)) {
+            *reinterpret_cast<float2 *>(o) = make_float2(a00, a01);
+            if (r1in) *reinterpret_cast<float2 *>(o + G.nx) = make_float2(a10, a11);
+        } else {
+            o[0] = a00;
+            if (c1in) o[1] = a01;
+            if (r1in) { o[G.nx] = a10; if (c1in) o[G.nx + 1] = a11; }
+        }
+        if (!c1in) { a01 = 0.f; a11 = 0.f; }
+        if (!r1in) { a10 = 0.f; a11 = 0.f; }
     }
     if (red) {
-        __shared__ float part[BP_ROWS];
-        float v = inside ? acc * acc : 0.f;
+        __shared__ float part[4];
+        float v = a00 * a00 + a01 * a01 + a10 * a10 + a11 * a11;
         v = warp_sum(v);
-        if (threadIdx.x == 0) part[threadIdx.y] = v;
+        if (lane == 0) part[warp] = v;
         __syncthreads();
-        if (threadIdx.y == 0 && threadIdx.x == 0) {
-            float s = 0.f;
-#pragma unroll
-            for (int i = 0; i < BP_ROWS; ++i) s += part[i];
-            atomicAdd(red + prob, (double)s);
-        }
+        if (threadIdx.x == 0) atomicAdd(red + prob, (double)(part[0] + part[1] + part[2] + part[3]));
     }
 }
 

@@ -32,6 +32,7 @@ struct tnlm_handle {
     int nx = 0, ny = 0, n_phase = 0, window = 0, patch = 0;
     float h = 0.f, mu = 0.f;
     bool has_geom = false;
+    bool fan_poly = true;   // every pixel is seen within +-45 degrees of the central ray: polynomial atan
     Geom G{};
     SweepParams R{};
     std::vector<SweepShape> shapes;   // launchable sweep shapes for this (window, patch)
@@ -267,6 +268,11 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         G.pix = (float)g.pixel_mm;
         G.sdd_over_pitch = (float)(g.sdd_mm / g.bin_pitch_mm);
         G.bin_centre = (float)(0.5 * (g.n_bins - 1) - g.bin_offset);
+        {   // largest |tan(fan angle)| of any point of the image, seen from any source position
+            const double hx = 0.5 * nx * g.pixel_mm, hy = 0.5 * ny * g.pixel_mm;
+            const double rmax = std::sqrt(hx * hx + hy * hy) + g.pixel_mm;
+            H->fan_poly = rmax / std::sqrt(std::fmax(g.sid_mm * g.sid_mm - rmax * rmax, 1e-30)) < 0.95;
+        }
         G.hw_scale = (float)(1.02 * g.pixel_mm * 0.70710678118654752 * g.sdd_mm / g.bin_pitch_mm);
         std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views;
         build_tables(g, nx, ny, n_phase, tab, rng, views);
@@ -354,8 +360,9 @@ static int launch_project(tnlm_handle *H, const float *img, const float *y, cons
 }
 static int launch_backproject(tnlm_handle *H, const float *sino, float *img, double *red, int n_slices, cudaStream_t st)
 {
-    dim3 grid((H->nx + 31) / 32, (H->ny + BP_ROWS - 1) / BP_ROWS, n_slices * H->n_phase);
-    backproject_kernel<<<grid, dim3(32, BP_ROWS), 0, st>>>(H->G, H->d_tab, H->d_rng, H->d_views, sino, img, red);
+    dim3 grid((H->nx + 15) / 16, (H->ny + 31) / 32, n_slices * H->n_phase);
+    if (H->fan_poly) backproject_kernel<true><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
+    else backproject_kernel<false><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
     LAUNCHED(H);
     return TNLM_OK;
 }
