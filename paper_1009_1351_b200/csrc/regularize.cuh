@@ -261,11 +261,14 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     __syncwarp();
 
     // ---- the window: items (dr, 4 consecutive dc), accumulators in registers
-    float Z[RB][C], A[RB][C];
+    // (column pairs: the vertical sums, exponents and accumulations issue as packed f32x2 instructions,
+    // which halves their issue slots; the FP32 pipe does the same lane work either way)
+    float2 Z[RB][C / 2], A[RB][C / 2];
 #pragma unroll
     for (int rr = 0; rr < RB; ++rr)
 #pragma unroll
-        for (int c = 0; c < C; ++c) { Z[rr][c] = 0.f; A[rr][c] = 0.f; }
+        for (int cp = 0; cp < C / 2; ++cp) { Z[rr][cp] = make_float2(0.f, 0.f); A[rr][cp] = make_float2(0.f, 0.f); }
+    const float2 negc2 = make_float2(p.neg_c, p.neg_c), neg1 = make_float2(-1.f, -1.f);
 
     // stored-weight chunk of this warp: [W*W][RB][128] halves
     constexpr size_t WSTRIDE = (size_t)RB * SW_TW;         // halves per offset
@@ -284,13 +287,15 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
         if (!STORE_W && okmask == 0) continue;     // (stored planes must be written even when all-zero)
         for (int dcg = 0; dcg < ng; ++dcg) {
             const int dc0 = -a + G * dcg;
-            float D[G][C], ring[G][C][RING];
+            float2 D[G][C / 2], ring[G][C / 2][RING];
 #pragma unroll
             for (int gg = 0; gg < G; ++gg)
 #pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    const int col = c0 + c + dc0 + gg;
-                    D[gg][c] = (dc0 + gg <= a && (unsigned)col < (unsigned)nx) ? 0.f : p.big_d;
+                for (int cp = 0; cp < C / 2; ++cp) {
+                    const int col = c0 + 2 * cp + dc0 + gg;
+                    const bool in_win = dc0 + gg <= a;
+                    D[gg][cp].x = (in_win && (unsigned)col < (unsigned)nx) ? 0.f : p.big_d;
+                    D[gg][cp].y = (in_win && (unsigned)(col + 1) < (unsigned)nx) ? 0.f : p.big_d;
                 }
             const float4 *__restrict__ gip = reinterpret_cast<const float4 *>(sGi + lr0 * GIW) + lane;
             const float4 *__restrict__ gjp = reinterpret_cast<const float4 *>(myGj + (lr0 + dr + a) * GJW) + lane + dcg;
@@ -311,7 +316,8 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                     const float4 v = gjp[s * (GJW / 4) + k];
                     gj_[4 * k] = v.x; gj_[4 * k + 1] = v.y; gj_[4 * k + 2] = v.z; gj_[4 * k + 3] = v.w;
                 }
-                float uj_[4 * NUJ], K_[C];
+                float uj_[4 * NUJ];
+                float2 K_[C / 2];
                 if (s >= 2 * PB) {                 // this step completes the window of pixel row rr
                     const int rr = s - 2 * PB;
                     // rows whose pixel or candidate row is outside the image get K = -huge: weight 0
@@ -322,8 +328,8 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         uj_[4 * k] = v.x; uj_[4 * k + 1] = v.y; uj_[4 * k + 2] = v.z; uj_[4 * k + 3] = v.w;
                     }
                     const float4 kv = kp[rr * (SW_TW / 4)];
-                    K_[0] = ok ? kv.x : -1.0e30f; K_[1] = ok ? kv.y : -1.0e30f;
-                    K_[2] = ok ? kv.z : -1.0e30f; K_[3] = ok ? kv.w : -1.0e30f;
+                    K_[0].x = ok ? kv.x : -1.0e30f; K_[0].y = ok ? kv.y : -1.0e30f;
+                    K_[1].x = ok ? kv.z : -1.0e30f; K_[1].y = ok ? kv.w : -1.0e30f;
                 }
 #pragma unroll
                 for (int gg = 0; gg < G; ++gg) {
@@ -341,24 +347,25 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         h = fmaf(-sd[c - 1], sd[c - 1], h);
                         H[c] = h;
                     }
+                    float2 e_[C / 2];
 #pragma unroll
-                    float e_[C];
-#pragma unroll
-                    for (int c = 0; c < C; ++c) {
-                        D[gg][c] += H[c];
+                    for (int cp = 0; cp < C / 2; ++cp) {
+                        const float2 H2 = make_float2(H[2 * cp], H[2 * cp + 1]);
+                        D[gg][cp] = __fadd2_rn(D[gg][cp], H2);
                         if (s >= 2 * PB) {
                             const int rr = s - 2 * PB;
-                            const float e = fast_ex2(fmaf(D[gg][c], p.neg_c, K_[c]));
-                            if (STORE_W) e_[c] = e;
-                            Z[rr][c] += e;
-                            A[rr][c] = fmaf(e, uj_[c + gg], A[rr][c]);
-                            D[gg][c] -= (PB > 0) ? ring[gg][c][s % RING] : H[c];
+                            const float2 t2 = __ffma2_rn(D[gg][cp], negc2, K_[cp]);
+                            const float2 e2 = make_float2(fast_ex2(t2.x), fast_ex2(t2.y));
+                            if (STORE_W) e_[cp] = e2;
+                            Z[rr][cp] = __fadd2_rn(Z[rr][cp], e2);
+                            A[rr][cp] = __ffma2_rn(e2, make_float2(uj_[2 * cp + gg], uj_[2 * cp + gg + 1]), A[rr][cp]);
+                            D[gg][cp] = __ffma2_rn((PB > 0) ? ring[gg][cp][s % RING] : H2, neg1, D[gg][cp]);
                         }
-                        ring[gg][c][s % RING] = H[c];
+                        ring[gg][cp][s % RING] = H2;
                     }
                     if (STORE_W && s >= 2 * PB) {  // one predicated 8-byte store: 4 bf16 weights of row rr, offset gg
                         const int rr = s - 2 * PB;
-                        const __nv_bfloat162 lo = __floats2bfloat162_rn(e_[0], e_[1]), hi = __floats2bfloat162_rn(e_[2], e_[3]);
+                        const __nv_bfloat162 lo = __floats2bfloat162_rn(e_[0].x, e_[0].y), hi = __floats2bfloat162_rn(e_[1].x, e_[1].y);
                         uint2 pk;
                         pk.x = *reinterpret_cast<const unsigned *>(&lo);
                         pk.y = *reinterpret_cast<const unsigned *>(&hi);
@@ -377,8 +384,10 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             const bool valid = (r0 + rr < ny) && (c0 + c < nx);
-            const bool bad = valid && !(Z[rr][c] < p.z_limit);
-            A[rr][c] = A[rr][c] / Z[rr][c];
+            float &Arc = (c & 1) ? A[rr][c >> 1].y : A[rr][c >> 1].x;
+            const float Zrc = (c & 1) ? Z[rr][c >> 1].y : Z[rr][c >> 1].x;
+            const bool bad = valid && !(Zrc < p.z_limit);
+            Arc = Arc / Zrc;
             unsigned m = __ballot_sync(0xffffffffu, bad);
             while (m) {
                 const int L = __ffs(m) - 1;
@@ -387,7 +396,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                 __syncwarp();                      // the fast path's stores to this pixel come first
                 const float v = exact_side_ratio<PB>(sGi, myGj, myUj, GJW, UJW, lr0 + rr, C * L + c, r0 + rr,
                                                      tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane, wpix, WSTRIDE);
-                if (lane == L) A[rr][c] = v;
+                if (lane == L) Arc = v;
             }
         }
 
@@ -395,7 +404,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     if (side == 1) {
 #pragma unroll
         for (int rr = 0; rr < RB; ++rr)
-            reinterpret_cast<float4 *>(myK)[rr * (SW_TW / 4) + lane] = make_float4(A[rr][0], A[rr][1], A[rr][2], A[rr][3]);
+            reinterpret_cast<float4 *>(myK)[rr * (SW_TW / 4) + lane] = make_float4(A[rr][0].x, A[rr][0].y, A[rr][1].x, A[rr][1].y);
     }
     __syncthreads();
     if (side == 0) {
@@ -412,7 +421,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 #pragma unroll
             for (int c = 0; c < C; ++c) {
                 const float gc = sGi[(lr0 + rr + PB) * GIW + C * lane + PB + c];
-                v[c] = fmaf(p.c_nb, A[rr][c] + on[c], p.c_self * gc);
+                v[c] = fmaf(p.c_nb, ((c & 1) ? A[rr][c >> 1].y : A[rr][c >> 1].x) + on[c], p.c_self * gc);
                 if (p.clip) v[c] = fmaxf(v[c], 0.f);
             }
             if (vec) {
