@@ -111,6 +111,12 @@ int tnlm_regularize_step(tnlm_handle *handle, const float *g, int m2, float *f_o
 int tnlm_reconstruct(tnlm_handle *handle, const float *y, const float *w, const float *f0,
                      int k_outer, int m1, int m2, float *f_out, int n_slices, void *stream);
 
+/* Step 1 of the "TNLM Algorithm": f0 = the filtered backprojection of ALL
+ * projections of ALL n_phase phases (equiangular fan-beam FBP, ramp filter, views weighted by the
+ * trapezoid rule over the sorted union of all source angles), the same image written to every
+ * phase.  y [S][N][V][B] -> f0 [S][N][ny][nx]; feed it to tnlm_reconstruct as `f0`. */
+int tnlm_fbp_init(tnlm_handle *handle, const float *y, float *f0, int n_slices, void *stream);
+
 /* Same operations with HOST buffers: host->device copies, the device path above, the
  * device->host copy of the result, and a stream synchronise, all inside the call. */
 int tnlm_regularize_step_host(tnlm_handle *handle, const float *g_host, int m2, float *f_out_host,

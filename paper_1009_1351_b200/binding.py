@@ -14,7 +14,7 @@ STATUS = {0: "TNLM_OK", 1: "TNLM_INVALID_ARG", 2: "TNLM_CUDA_ERROR", 3: "TNLM_AL
 EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "tnlm_cgls_step",
            "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
            "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version",
-           "tnlm_profile_sweeps", "tnlm_sweep_times"]
+           "tnlm_profile_sweeps", "tnlm_sweep_times", "tnlm_fbp_init"]
 
 KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply"}
 
@@ -74,6 +74,7 @@ def library():
         L.tnlm_launch_count.restype = C.c_longlong
         L.tnlm_version.restype = C.c_char_p
         L.tnlm_profile_sweeps.argtypes = [P, I]
+        L.tnlm_fbp_init.argtypes = [P, P, P, I, P]
         L.tnlm_sweep_times.argtypes = [P, C.POINTER(C.c_float), C.POINTER(I), I, C.POINTER(I)]
         _LIB = L
     return _LIB
@@ -160,6 +161,12 @@ def backproject(h: Handle, sino, img, stream=None):
     S = _slices(h, img, h.n_phase * h.nx * h.ny)
     h.check(library().tnlm_backproject(h.ptr, _dev(sino, "sino"), _dev(img, "img"), S, _stream(stream)))
     return img
+
+
+def fbp_init(h: Handle, y, f0, stream=None):
+    S = _slices(h, f0, h.n_phase * h.nx * h.ny)
+    h.check(library().tnlm_fbp_init(h.ptr, _dev(y, "y"), _dev(f0, "f0"), S, _stream(stream)))
+    return f0
 
 
 def cgls_step(h: Handle, f_in, y, w, m1, g_out, stream=None):

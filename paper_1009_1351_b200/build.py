@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtnlm.so")
 SOURCES = ["tnlm_api.cu"]
-DEPS = ["tnlm_api.cu", "common.cuh", "projector.cuh", "cgls.cuh", "regularize.cuh",
+DEPS = ["tnlm_api.cu", "common.cuh", "projector.cuh", "cgls.cuh", "regularize.cuh", "fbp.cuh",
         os.path.join("..", "..", "include", "tnlm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

@@ -13,6 +13,7 @@
 #include "../../include/tnlm.h"
 #include "cgls.cuh"
 #include "common.cuh"
+#include "fbp.cuh"
 #include "projector.cuh"
 #include "regularize.cuh"
 
@@ -42,6 +43,10 @@ struct tnlm_handle {
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
     float4 *d_views = nullptr;
+    // FBP initialisation (fbp.cuh): ramp filter table, cosine weights, view weights; filtered sinograms
+    double *d_fbp_g = nullptr;
+    float *d_fbp_cosw = nullptr, *d_fbp_wv = nullptr;
+    float *d_fbp_q = nullptr;
     // workspace, sized for ws_slices
     int ws_slices = 0;
     float *d_s = nullptr, *d_t = nullptr, *d_g = nullptr, *d_f = nullptr;  // images
@@ -287,6 +292,41 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
             tnlm_destroy(H);
             return fail(nullptr, TNLM_ALLOC_FAILED, "device allocation failed (geometry tables)");
         }
+        {   // FBP tables (double precision on the host)
+            const int B = g.n_bins, M = n_phase * g.n_views;
+            const double dgam = g.bin_pitch_mm / g.sdd_mm, two_pi = 6.283185307179586476925;
+            std::vector<double> gk(B);
+            std::vector<float> cosw(B), wv(M);
+            for (int k = 0; k < B; ++k) {
+                const double sk = std::sin(k * dgam);
+                gk[k] = (k == 0) ? dgam / (8.0 * dgam * dgam) : ((k & 1) ? -dgam / (2.0 * 9.869604401089358 * sk * sk) : 0.0);
+                cosw[k] = (float)(g.sid_mm * std::cos((k - 0.5 * (B - 1) + g.bin_offset) * dgam));
+            }
+            // trapezoid weights over the sorted cyclic union of all source angles
+            std::vector<std::pair<double, int>> ord(M);
+            for (int j = 0; j < M; ++j) {
+                double bj = std::fmod(g.angles_rad[j], two_pi);
+                if (bj < 0) bj += two_pi;
+                ord[j] = std::make_pair(bj, j);
+            }
+            std::stable_sort(ord.begin(), ord.end(), [](const std::pair<double, int> &x, const std::pair<double, int> &y) { return x.first < y.first; });
+            for (int t = 0; t < M; ++t) {
+                const double nxt = (t + 1 < M) ? ord[t + 1].first : ord[0].first + two_pi;
+                const double prv = (t > 0) ? ord[t - 1].first : ord[M - 1].first - two_pi;
+                wv[ord[t].second] = (float)(0.5 * (nxt - prv));
+            }
+            bool ok2 = cudaMalloc(&H->d_fbp_g, B * sizeof(double)) == cudaSuccess &&
+                       cudaMalloc(&H->d_fbp_cosw, B * sizeof(float)) == cudaSuccess &&
+                       cudaMalloc(&H->d_fbp_wv, M * sizeof(float)) == cudaSuccess;
+            if (ok2) ok2 = cudaMemcpy(H->d_fbp_g, gk.data(), B * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess &&
+                           cudaMemcpy(H->d_fbp_cosw, cosw.data(), B * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess &&
+                           cudaMemcpy(H->d_fbp_wv, wv.data(), M * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess;
+            if (!ok2) {
+                cudaGetLastError();
+                tnlm_destroy(H);
+                return fail(nullptr, TNLM_ALLOC_FAILED, "device allocation failed (FBP tables)");
+            }
+        }
         H->has_geom = true;
     }
     *out = H;
@@ -295,7 +335,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
 
 static void free_ws(tnlm_handle *H)
 {
-    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_r, &H->d_rw, &H->d_q, &H->d_yh, &H->d_wh};
+    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_fbp_q, &H->d_r, &H->d_rw, &H->d_q, &H->d_yh, &H->d_wh};
     for (float **b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     H->ws_slices = 0;
 }
@@ -307,6 +347,9 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
     if (H->d_wts) cudaFree(H->d_wts);
+    if (H->d_fbp_g) cudaFree(H->d_fbp_g);
+    if (H->d_fbp_cosw) cudaFree(H->d_fbp_cosw);
+    if (H->d_fbp_wv) cudaFree(H->d_fbp_wv);
     if (H->d_tab) cudaFree(H->d_tab);
     if (H->d_rng) cudaFree(H->d_rng);
     if (H->d_views) cudaFree(H->d_views);
@@ -382,6 +425,26 @@ extern "C" int tnlm_backproject(tnlm_handle *H, const float *sino, float *img, i
     if (rc) return rc;
     if (!img || !sino) return fail(H, TNLM_INVALID_ARG, "img and sino must not be NULL");
     return launch_backproject(H, sino, img, nullptr, n_slices, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------ FBP initialisation
+extern "C" int tnlm_fbp_init(tnlm_handle *H, const float *y, float *f0, int n_slices, void *stream)
+{
+    int rc = check_common(H, n_slices, true);
+    if (rc) return rc;
+    if (!y || !f0) return fail(H, TNLM_INVALID_ARG, "y and f0 must not be NULL");
+    if ((size_t)H->G.n_bins * sizeof(float) > 48 * 1024) return fail(H, TNLM_UNSUPPORTED, "more than 12288 detector bins");
+    if ((rc = ensure_ws(H, n_slices))) return rc;
+    if ((rc = need(H, &H->d_fbp_q, sino_count(H)))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int M = H->n_phase * H->G.n_views;
+    fbp_filter_kernel<<<dim3(M, n_slices), 256, H->G.n_bins * sizeof(float), st>>>(y, H->d_fbp_q, H->d_fbp_cosw, H->d_fbp_g,
+                                                                                      H->G.n_bins);
+    LAUNCHED(H);
+    fbp_backproject_kernel<<<dim3((H->nx + 31) / 32, (H->ny + 7) / 8, n_slices), dim3(32, 8), 0, st>>>(
+        H->G, H->d_views, H->d_fbp_wv, H->d_fbp_q, f0);
+    LAUNCHED(H);
+    return TNLM_OK;
 }
 
 // ------------------------------------------------------------------------------ CGLS

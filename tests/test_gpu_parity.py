@@ -291,6 +291,47 @@ def test_config4_window_full_size_on_sampled_pixels(T):
     assert rel(out.cpu().numpy().ravel()[pix], np.maximum(want, 0)) < STEP_TOL
 
 
+# ------------------------------------------------------------------------------ FBP initialisation
+@pytest.mark.parametrize("cfg", [workloads.config(1), small_geom_cfg(L=37, N=2, V=23, B=61),
+                                 workloads.Config("fbp", L=96, N=3, V=120, B=300, pitch=0.8, sid=400.0, sdd=800.0,
+                                                  I0=1e5, window=5, patch=3)],
+                         ids=["cfg1", "odd37", "fine96"])
+def test_fbp_init_matches_oracle(T, cfg):
+    # step 1 of the TNLM algorithm: FBP of all projections of all phases, same image per phase
+    from oracle import fbp
+    torch, tn = T
+    h, og = handles(tn, cfg)
+    y = workloads.make_inputs(cfg)["y"][0].astype(np.float32)
+    f0 = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.fbp_init(h, dev(torch, y), f0)
+    want = fbp.fbp_init(og, y, cfg.L, cfg.L)
+    got = f0.cpu().numpy()
+    assert all(np.array_equal(got[0], got[i]) for i in range(cfg.N))
+    assert rel(got, want) < STEP_TOL
+    assert np.abs(got - want).max() < 1e-4 * np.abs(want).max()
+
+
+def test_reconstruct_from_fbp_start_matches_oracle(T):
+    from oracle import fbp
+    torch, tn = T
+    cfg = workloads.config(1)
+    h, og = handles(tn, cfg)
+    inp = workloads.make_inputs(cfg)
+    y, w = inp["y"][0].astype(np.float32), inp["w"][0].astype(np.float32)
+    f0 = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.fbp_init(h, dev(torch, y), f0)
+    out = torch.empty_like(f0)
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), f0, 2, cfg.m1, cfg.m2, out)
+    want0 = fbp.fbp_init(og, y, cfg.L, cfg.L)
+    want = oracle.reconstruct(og, y, w, want0, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 2, cfg.m1, cfg.m2)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL * 3
+    # the FBP start is closer to the phantom than the zero start after the same two outer iterations
+    z = torch.empty_like(f0)
+    tn.reconstruct(h, dev(torch, y), dev(torch, w), None, 2, cfg.m1, cfg.m2, z)
+    ph = inp["phantom"][0]
+    assert rel(out.cpu().numpy(), ph) < rel(z.cpu().numpy(), ph)
+
+
 # ------------------------------------------------------------------------------ whole iteration
 def test_reconstruct_config1_matches_oracle(T):
     torch, tn = T
