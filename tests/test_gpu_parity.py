@@ -172,6 +172,8 @@ def noisy_stack(N, ny, nx, seed, sigma=0.002):
     (2, 33, 65, 7, 1, 0.004, 0.5, 3),      # N=2: both neighbours are the same phase; patch 1
     (1, 50, 50, 3, 9, 0.02, 0.3, 2),       # N=1 degenerate self-NLM; patch 9
     (5, 30, 30, 1, 3, 0.01, 0.4, 2),       # window 1
+    (2, 40, 50, 31, 9, 0.02, 0.2, 2),      # the compiled maxima: window 31, patch 9 (stored weights, nx % 4 != 0)
+    (3, 150, 260, 9, 3, 0.006, 0.15, 3),   # three column tiles, ragged last tile, stored weights
 ])
 def test_regularize_step_matches_oracle(T, N, ny, nx, W, d, h, mu, m2):
     torch, tn = T
