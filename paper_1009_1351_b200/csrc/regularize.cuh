@@ -478,6 +478,9 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
 // over, nothing else synchronises.  u_j of both neighbours is staged with its halo in shared
 // memory, zero-filled outside the image (excluded candidates carry weight 0 in the chunks).
 // grid.x = (S*N) * ceil(ny / rb) * tiles_x; block = 32 * (rb + 1).
+// Measured ceiling (round-1 working notes): streaming the same 322 MB by bulk copies alone, no arithmetic,
+// takes 65 us (4.9 TB/s) for any stage size 2.5-31 KB and ring depth 2-8; a grid-stride LDG.128 read
+// reaches 5.6 TB/s, but an 8-byte-per-lane register-pipelined variant of this kernel ran at 151 us.
 constexpr int AP_SO = 4;         // offsets (consecutive dc of one dr) per stage
 constexpr int AP_NS_MAX = 8;     // stages in flight: p.ap_ns, chosen per launch (wave quantisation vs bytes in flight)
 __host__ __device__ inline int apply_uw(int window) { return 124 + 4 * ((window + 3) / 4 + 1); }

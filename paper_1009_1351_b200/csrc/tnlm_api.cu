@@ -570,7 +570,7 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
         const long long occ = std::min<long long>((long long)(H->smem_per_sm / (sm + 1024)), 2048 / threads);
         if (occ < 1) continue;
         const long long cap = occ * H->n_sm, waves = (ctas + cap - 1) / cap;
-        const double eff = (double)ctas / (double)(waves * cap) + 1e-3 * ns;     // ties: deeper ring
+        const double eff = (double)ctas / (double)(waves * cap) - 1e-3 * (double)waves + 1e-5 * ns;   // ties: fewer waves, then deeper ring
         if (eff > best_eff) { best_eff = eff; R.ap_ns = ns; smem = sm; }
     }
     if (best_eff < 0.0) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
