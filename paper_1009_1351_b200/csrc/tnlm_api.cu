@@ -256,6 +256,10 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         H->apply_smem = std::min(apply_smem_bytes(window, 10, AP_NS_MAX), (size_t)prop.sharedMemPerBlockOptin);   // rb <= 10
         ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)H->apply_smem);
+        // ask for the largest shared-memory carveout so that the ring-depth choice below decides the occupancy
+        if (ce == cudaSuccess)
+            ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      cudaSharedmemCarveoutMaxShared);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
     }
     H->n_sm = prop.multiProcessorCount;
