@@ -340,10 +340,24 @@ def time_recon(tn, torch, args):
     s = a.elapsed_time(b) * 1e-3 / reps
     ph = torch.from_numpy(inp["phantom"].astype(np.float32)).cuda()
     err = float(((out - ph).norm() / ph.norm()).item())
+    # quality figures of the paper's section 3 on the synthetic phantom (Eq. 10, Eq. 11): TNLM result vs the
+    # all-phase FBP image (step 1 of the algorithm, tnlm_fbp_init), mean over the phases
+    from workloads import quality
+    fbp = torch.empty_like(out)
+    tn.fbp_init(h, y, fbp, st)
+    torch.cuda.synchronize()
+    rec, fb, truth = out[0].cpu().numpy(), fbp[0].cpu().numpy(), inp["phantom"][0]
+    q = {"snr_db_tnlm": 0.0, "snr_db_fbp_all_phases": 0.0, "cnr_tumour_tnlm": 0.0, "cnr_tumour_fbp_all_phases": 0.0}
+    for i in range(cfg.N):
+        sig, bg = quality.tumour_rois(truth[i])
+        q["snr_db_tnlm"] += quality.snr_db(rec[i], truth[i]) / cfg.N
+        q["snr_db_fbp_all_phases"] += quality.snr_db(fb[i], truth[i]) / cfg.N
+        q["cnr_tumour_tnlm"] += quality.cnr(rec[i], sig, bg) / cfg.N
+        q["cnr_tumour_fbp_all_phases"] += quality.cnr(fb[i], sig, bg) / cfg.N
     return {"metric": "s per 10-phase slice recon", "value": s, "unit": "s", "higher_is_better": False,
             "workload": "BASELINE.json configs[3]: 512x512x10, 60 views x 888 bins, W=15 d=7, "
                         f"K={cfg.K} m1={cfg.m1} m2={cfg.m2}, f0=0",
-            "gpu_launches": int((h.launch_count - n0) // reps), "rel_l2_to_phantom": err,
+            "gpu_launches": int((h.launch_count - n0) // reps), "rel_l2_to_phantom": err, "quality": q,
             "paper_context": "40-90 s per 10-phase slice on a Tesla C1060 (PAPER.md:L15), other workload"}
 
 
