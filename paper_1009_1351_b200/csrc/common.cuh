@@ -19,7 +19,8 @@ struct __align__(16) RayEntry {
 };
 struct __align__(8) RayRange {
     short lo, hi;      // inclusive range of rows (steep) / columns (shallow) to walk; empty if hi < lo
-    int steep;
+    short ilo, ihi;    // sub-range in which both touched cells are certainly inside the image (no bounds tests);
+                       // empty if ihi < ilo
 };
 
 struct Geom {

@@ -72,30 +72,36 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
     if (ray < nray) {
         const RayEntry e = tab[(size_t)phase * nray + ray];
         const RayRange rg = rng[(size_t)phase * nray + ray];
-        const float *__restrict__ im = img + (size_t)prob * G.nx * G.ny;
         const float alen = fabsf(e.len);
         float acc0 = 0.f, acc1 = 0.f;
-        float qf = (float)rg.lo;
-        if (rg.steep) {
-            const int nx = G.nx;
-            const float *__restrict__ row = im + (size_t)rg.lo * nx;
-#pragma unroll 4
-            for (int q = rg.lo; q <= rg.hi; ++q, qf += 1.0f, row += nx) {
+        // steep rays walk the rows of the image, shallow rays the rows of the transposed image
+        const bool steep = e.len > 0.f;
+        const int n_minor = steep ? G.nx : G.ny;             // length of a walked row
+        const float *__restrict__ base = (steep ? img : imgT) + (size_t)prob * G.nx * G.ny;
+        auto edge = [&](int q0, int q1) {                      // rows in which a touched cell may be outside
+            float qf = (float)q0;
+            const float *__restrict__ row = base + (size_t)q0 * n_minor;
+            for (int q = q0; q <= q1; ++q, qf += 1.0f, row += n_minor) {
                 int c0; float w0, w1;
                 ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
-                if ((unsigned)c0 < (unsigned)nx) acc0 = fmaf(w0, __ldg(row + c0), acc0);
-                if ((unsigned)(c0 + 1) < (unsigned)nx) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
+                if ((unsigned)c0 < (unsigned)n_minor) acc0 = fmaf(w0, __ldg(row + c0), acc0);
+                if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
             }
-        } else {                                   // shallow: the same walk over the rows of the transposed image
-            const int ny = G.ny;
-            const float *__restrict__ row = imgT + (size_t)prob * G.nx * ny + (size_t)rg.lo * ny;
+        };
+        if (rg.ihi >= rg.ilo) {
+            edge(rg.lo, rg.ilo - 1);
+            float qf = (float)rg.ilo;
+            const float *__restrict__ row = base + (size_t)rg.ilo * n_minor;
 #pragma unroll 4
-            for (int q = rg.lo; q <= rg.hi; ++q, qf += 1.0f, row += ny) {
+            for (int q = rg.ilo; q <= rg.ihi; ++q, qf += 1.0f, row += n_minor) {
                 int c0; float w0, w1;
                 ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
-                if ((unsigned)c0 < (unsigned)ny) acc0 = fmaf(w0, __ldg(row + c0), acc0);
-                if ((unsigned)(c0 + 1) < (unsigned)ny) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
+                acc0 = fmaf(w0, __ldg(row + c0), acc0);
+                acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
             }
+            edge(rg.ihi + 1, rg.hi);
+        } else {
+            edge(rg.lo, rg.hi);
         }
         const float p = acc0 + acc1;
         const size_t o = (size_t)prob * nray + ray;

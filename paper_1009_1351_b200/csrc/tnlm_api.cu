@@ -137,7 +137,23 @@ static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, st
                     hi = -1;
                 }
                 RayRange r;
-                r.lo = (short)lo; r.hi = (short)hi; r.steep = steep ? 1 : 0;
+                r.lo = (short)lo; r.hi = (short)hi;
+                // interior: lo(q) = m*q + plo within [0.5, n_minor - 2.5], so that the fp32 floor c0 and c0+1
+                // are inside whatever the rounding; lo(q) is linear in q, so the rows form one interval
+                r.ilo = 0; r.ihi = -1;
+                if (hi >= lo) {
+                    const double plo = p0 + std::fmin(m, 0.0), a0 = 0.5, a1 = (double)n_minor - 2.5;
+                    double q0 = (double)lo, q1 = (double)hi;
+                    if (e.m != 0.f) {
+                        double t0 = (a0 - plo) / m, t1 = (a1 - plo) / m;
+                        if (t0 > t1) std::swap(t0, t1);
+                        q0 = std::fmax(q0, std::ceil(t0) + 1.0);
+                        q1 = std::fmin(q1, std::floor(t1) - 1.0);
+                    } else if (!(plo >= a0 && plo <= a1)) {
+                        q1 = q0 - 1.0;
+                    }
+                    if (q1 >= q0) { r.ilo = (short)q0; r.ihi = (short)q1; }
+                }
                 tab[((size_t)i * V + v) * B + k] = e;
                 rng[((size_t)i * V + v) * B + k] = r;
             }
