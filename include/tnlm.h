@@ -42,6 +42,13 @@
  *   device.  `_host` entry points copy in, run, copy out and synchronise `stream` before
  *   returning.  A handle must not be used from two streams or threads at once.
  *
+ * Stored weights and tuning knobs
+ *   The weights belong to g^(k) and are the same in all m2 sweeps (L162), so for m2 > 1 the first
+ *   sweep stores them (bf16, 2*W^2*2 bytes per pixel, handle-owned) and the later sweeps stream them
+ *   (L206 "reusing this factor ... instead of recomputing").  Environment variables read per call:
+ *   TNLM_WEIGHT_CACHE_MB (default 16384; larger needs, or 0, make every sweep recompute in fp32),
+ *   TNLM_SWEEP_SHAPE="rb,nb" and TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).
+ *
  * Errors
  *   Every call returns a tnlm_status; nothing throws, exits or falls back to the CPU.
  *   tnlm_last_error(handle) gives a handle-owned message for the last failing call.
