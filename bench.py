@@ -172,11 +172,13 @@ def workload_config(cfg, n_gpus):
 # ---------------------------------------------------------------------------------------- our arm
 def run_ours(args):
     import torch
-    import paper_1009_1351_b200 as tn
-
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if local == 0:
+        from paper_1009_1351_b200 import build
+        build.build()                # no-op when libtnlm.so is newer than its sources
+    import paper_1009_1351_b200 as tn
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; libtnlm has no CPU fallback")
     torch.cuda.set_device(local)
@@ -190,6 +192,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    barrier()                                        # (local rank 0 may just have built the library)
     cfg, g_np = cfg2_input(1 + rank)                 # one independent slice per rank
     n_px_step = g_np.size * cfg.m2                   # pixel updates of one step on this rank
     h = tn.create(None, cfg.L, cfg.L, cfg.N, cfg.window, cfg.patch, cfg.h, cfg.mu)

@@ -23,6 +23,8 @@ def rel(a, b):
 @pytest.fixture(scope="module")
 def T():
     import torch
+    from paper_1009_1351_b200 import build
+    build.build()                    # no-op when libtnlm.so is newer than its sources
     import paper_1009_1351_b200 as tn
     assert torch.cuda.is_available()
     return torch, tn
