@@ -310,6 +310,7 @@ def run_ours(args):
 
     if world == 1 and not args.no_recon:
         line["recon"] = time_recon(tn, torch, args)
+        line["recon_low_mas"] = time_recon(tn, torch, args, which=3)
     if world == 1 and not args.no_cpu:
         v, sweeps, dt, cores = time_oracle(cfg, g_np.astype(np.float64), args.cpu_budget)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -320,10 +321,11 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def time_recon(tn, torch, args):
+def time_recon(tn, torch, args, which=4):
     """Second half of BASELINE.json's metric: seconds per 10-phase slice reconstruction
-    (tnlm_reconstruct), on configs[3] (512x512x10, 60 views, 888 bins, W=15, d=7, 30 outer)."""
-    cfg = workloads.config(4)
+    (tnlm_reconstruct), on configs[3] (512x512x10, 60 views, 888 bins, W=15, d=7, 30 outer) or, which=3,
+    configs[2] (360 views, W=11, d=5, 20 outer, 5 CGLS steps)."""
+    cfg = workloads.config(which)
     inp = workloads.make_inputs(cfg)
     h = tn.create(tn.Geometry(**workloads.geometry_kwargs(cfg)), cfg.L, cfg.L, cfg.N, cfg.window, cfg.patch,
                   cfg.h, cfg.mu)
@@ -334,7 +336,7 @@ def time_recon(tn, torch, args):
     tn.reconstruct(h, y, w, None, 2, cfg.m1, cfg.m2, out, st)
     torch.cuda.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps, n0 = 3, h.launch_count
+    reps, n0 = (3 if which == 4 else 1), h.launch_count
     a.record(st)
     for _ in range(reps):
         tn.reconstruct(h, y, w, None, cfg.K, cfg.m1, cfg.m2, out, st)
@@ -358,8 +360,8 @@ def time_recon(tn, torch, args):
         q["cnr_tumour_tnlm"] += quality.cnr(rec[i], sig, bg) / cfg.N
         q["cnr_tumour_fbp_all_phases"] += quality.cnr(fb[i], sig, bg) / cfg.N
     return {"metric": "s per 10-phase slice recon", "value": s, "unit": "s", "higher_is_better": False,
-            "workload": "BASELINE.json configs[3]: 512x512x10, 60 views x 888 bins, W=15 d=7, "
-                        f"K={cfg.K} m1={cfg.m1} m2={cfg.m2}, f0=0",
+            "workload": f"BASELINE.json configs[{which - 1}]: {cfg.L}x{cfg.L}x{cfg.N}, {cfg.V} views x {cfg.B} bins, "
+                        f"W={cfg.window} d={cfg.patch}, K={cfg.K} m1={cfg.m1} m2={cfg.m2}, f0=0",
             "gpu_launches": int((h.launch_count - n0) // reps), "rel_l2_to_phantom": err, "quality": q,
             "paper_context": "40-90 s per 10-phase slice on a Tesla C1060 (PAPER.md:L15), other workload"}
 
