@@ -150,6 +150,11 @@ typedef enum {
 int tnlm_profile_sweeps(tnlm_handle *handle, int enable);
 int tnlm_sweep_times(tnlm_handle *handle, float *ms, int *kind, int capacity, int *count);
 
+/* Measured FP32 (non-tensor) FMA peak of the current device in TFLOP/s (2 flops per FFMA): an
+ * 8-chain FFMA kernel on every SM, best of 3 timed launches on `stream` (synchronises).  The
+ * roofline denominator of the ALU-bound TNLM kernels; no handle needed. */
+int tnlm_fma_peak(double *tflops, void *stream);
+
 /* Number of CUDA kernels this handle has launched so far (for benchmark bookkeeping). */
 long long tnlm_launch_count(const tnlm_handle *handle);
 

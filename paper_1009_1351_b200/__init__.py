@@ -8,4 +8,4 @@ fallback: if the library is missing or no CUDA device is present the calls fail 
 """
 from .binding import (Geometry, Handle, TnlmError, cgls_step, create, lib_path, library,  # noqa: F401
                       backproject, project, reconstruct, regularize_step, reconstruct_host,
-                      regularize_step_host, version, profile_sweeps, sweep_times, fbp_init)
+                      regularize_step_host, version, profile_sweeps, sweep_times, fbp_init, fma_peak)

@@ -14,7 +14,7 @@ STATUS = {0: "TNLM_OK", 1: "TNLM_INVALID_ARG", 2: "TNLM_CUDA_ERROR", 3: "TNLM_AL
 EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "tnlm_cgls_step",
            "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
            "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version",
-           "tnlm_profile_sweeps", "tnlm_sweep_times", "tnlm_fbp_init"]
+           "tnlm_profile_sweeps", "tnlm_sweep_times", "tnlm_fbp_init", "tnlm_fma_peak"]
 
 KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply"}
 
@@ -75,6 +75,7 @@ def library():
         L.tnlm_version.restype = C.c_char_p
         L.tnlm_profile_sweeps.argtypes = [P, I]
         L.tnlm_fbp_init.argtypes = [P, P, P, I, P]
+        L.tnlm_fma_peak.argtypes = [C.POINTER(C.c_double), P]
         L.tnlm_sweep_times.argtypes = [P, C.POINTER(C.c_float), C.POINTER(I), I, C.POINTER(I)]
         _LIB = L
     return _LIB
@@ -187,6 +188,15 @@ def reconstruct(h: Handle, y, w, f0, k_outer, m1, m2, f_out, stream=None):
     h.check(library().tnlm_reconstruct(h.ptr, _dev(y, "y"), _dev(w, "w"), _dev(f0, "f0"), k_outer, m1, m2,
                                        _dev(f_out, "f_out"), S, _stream(stream)))
     return f_out
+
+
+def fma_peak(stream=None) -> float:
+    """Measured FP32 FMA peak of the current device, TFLOP/s."""
+    out = C.c_double(0.0)
+    rc = library().tnlm_fma_peak(C.byref(out), _stream(stream))
+    if rc != 0:
+        raise TnlmError(rc, (library().tnlm_last_error(None) or b"").decode())
+    return float(out.value)
 
 
 def profile_sweeps(h: Handle, enable: bool):

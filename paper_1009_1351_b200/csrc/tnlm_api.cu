@@ -637,6 +637,38 @@ static int prof_mark(tnlm_handle *H, int kind, bool begin, cudaStream_t st)
     return TNLM_OK;
 }
 
+extern "C" int tnlm_fma_peak(double *tflops, void *stream)
+{
+    if (!tflops) return TNLM_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    float *d = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (ce == cudaSuccess) ce = cudaMalloc(&d, sizeof(float));
+    if (ce == cudaSuccess) ce = cudaEventCreate(&e0);
+    if (ce == cudaSuccess) ce = cudaEventCreate(&e1);
+    const int blocks = n_sm * 8, iters = 2048;
+    double best = 0.0;
+    for (int rep = 0; rep < 4 && ce == cudaSuccess; ++rep) {        // first launch warms up
+        cudaEventRecord(e0, st);
+        fp32_probe_kernel<<<blocks, 256, 0, st>>>(d, 1.0001f, 0.5f, iters);
+        cudaEventRecord(e1, st);
+        ce = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 8 * 16 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (d) cudaFree(d);
+    if (ce != cudaSuccess) { cuda_fail(nullptr, ce, "tnlm_fma_peak"); return TNLM_CUDA_ERROR; }
+    *tflops = best;
+    return TNLM_OK;
+}
+
 extern "C" int tnlm_profile_sweeps(tnlm_handle *H, int enable)
 {
     if (!H) return TNLM_INVALID_ARG;
