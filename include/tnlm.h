@@ -38,16 +38,27 @@
  *
  * Execution
  *   Device entry points enqueue work on `stream` (a cudaStream_t passed as void*, NULL = the
- *   legacy default stream) and return without synchronising; all scalars of CGLS stay on the
- *   device.  `_host` entry points copy in, run, copy out and synchronise `stream` before
- *   returning.  A handle must not be used from two streams or threads at once.
+ *   legacy default stream) and return without waiting for it; all scalars of CGLS stay on the
+ *   device.  The FIRST call that needs a workspace buffer of some kind, and any call with a larger
+ *   n_slices than seen before, allocates it with cudaMalloc inside the call, which synchronises
+ *   the device; tnlm_reserve does all of that up front, after which the enqueue calls never
+ *   allocate.  `_host` entry points copy in, run, copy out and synchronise `stream` before
+ *   returning.  A handle belongs to the CUDA device that was current at tnlm_create: every entry
+ *   point makes that device current for the call and restores the caller's; device pointers and
+ *   the stream must belong to it.  A handle must not be used from two streams or threads at once.
  *
  * Stored weights and tuning knobs
  *   The weights belong to g^(k) and are the same in all m2 sweeps (L162), so for m2 > 1 the first
  *   sweep stores them (bf16, 2*W^2*2 bytes per pixel, handle-owned) and the later sweeps stream them
- *   (L206 "reusing this factor ... instead of recomputing").  Environment variables read per call:
- *   TNLM_WEIGHT_CACHE_MB (default 16384; larger needs, or 0, make every sweep recompute in fp32),
- *   TNLM_SWEEP_SHAPE="rb,nb" and TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).
+ *   (L206 "reusing this factor ... instead of recomputing"); accumulation stays fp32.  Options, read
+ *   from the environment ONCE at tnlm_create and changed later with tnlm_set_option:
+ *   weight_cache_mb / TNLM_WEIGHT_CACHE_MB (default 16384; larger needs, or 0, make every sweep
+ *   recompute the weights in fp32), sweep_rb, sweep_nb / TNLM_SWEEP_SHAPE="rb,nb" and
+ *   apply_ns / TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).
+ *
+ * Value range
+ *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
+ *   finite for |u| < 2^17 (1.3e5; HU-scaled images are fine).  h must be <= 1e12.
  *
  * Errors
  *   Every call returns a tnlm_status; nothing throws, exits or falls back to the CPU.
@@ -133,22 +144,40 @@ int tnlm_reconstruct_host(tnlm_handle *handle, const float *y_host, const float 
                           int n_slices, void *stream);
 
 /* Message of the last failing call on this handle ("" if none); handle-owned, valid until the
- * next call on the handle.  NULL handle -> message of the last failed tnlm_create. */
+ * next call on the handle.  NULL handle -> message of the calling thread's last failed tnlm_create. */
 const char *tnlm_last_error(const tnlm_handle *handle);
 
-/* Per-launch device timing of the TNLM kernels (steps 3-5), for benchmarks and rooflines.
- * tnlm_profile_sweeps(handle, 1) makes every later tnlm_regularize_step / tnlm_reconstruct call
- * bracket each sweep kernel with a CUDA event pair on the call's stream (0 switches it off;
- * either call forgets the launches recorded so far).  tnlm_sweep_times waits for the recorded
- * launches, writes up to `capacity` durations (milliseconds, launch order) into the HOST arrays
- * ms[] and kind[] (a tnlm_kernel_kind), stores the number recorded in *count, and forgets them. */
+/* Allocate now everything a later tnlm_cgls_step / tnlm_regularize_step / tnlm_reconstruct call
+ * with up to n_slices slices, m1 CGLS steps and m2 sweeps would allocate on first use
+ * (host_entry_points != 0: also the staging buffers of the _host calls).  Synchronises the device. */
+int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_entry_points);
+
+/* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
+ * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns"; 0 restores the heuristic for the last three. */
+int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
+
+/* The CUDA device ordinal the handle was created on (-1 for a NULL handle). */
+int tnlm_device(const tnlm_handle *handle);
+
+/* Per-launch device timing of every kernel of the path, for benchmarks and rooflines.
+ * tnlm_profile_kernels(handle, 1) makes every later call bracket each kernel launch with a CUDA
+ * event pair on the call's stream (0 switches it off; either call forgets the launches recorded
+ * so far).  tnlm_kernel_times waits for the recorded launches, writes up to `capacity` durations
+ * (milliseconds, launch order) into the HOST arrays ms[] and kind[] (a tnlm_kernel_kind), stores
+ * the number recorded in *count, and forgets them. */
 typedef enum {
     TNLM_KERNEL_SWEEP = 0,       /* weights computed on the fly + one Gauss-Jacobi sweep (Eq. 3/8, Eq. 7) */
     TNLM_KERNEL_SWEEP_STORE = 1, /* the same, also storing the weights of g^(k) for sweeps 2..m2 */
-    TNLM_KERNEL_APPLY = 2        /* one Gauss-Jacobi sweep of Eq. (7) from the stored weights */
+    TNLM_KERNEL_APPLY = 2,       /* one Gauss-Jacobi sweep of Eq. (7) from the stored weights */
+    TNLM_KERNEL_PROJECT = 3,     /* forward projector P with the CGLS epilogue (L75, L109, L112) */
+    TNLM_KERNEL_BACKPROJECT = 4, /* backprojector P^T with the norm reduction (L79, L109, L124) */
+    TNLM_KERNEL_TRANSPOSE = 5,   /* transposed image copy read by the shallow rays of P */
+    TNLM_KERNEL_CGLS_VECTOR = 6, /* CGLS vector updates (L114-L126) and sqrt(w) */
+    TNLM_KERNEL_CLIP = 7,        /* positivity clip alone (m2 = 0) */
+    TNLM_KERNEL_FBP = 8          /* FBP initialisation kernels (L175) */
 } tnlm_kernel_kind;
-int tnlm_profile_sweeps(tnlm_handle *handle, int enable);
-int tnlm_sweep_times(tnlm_handle *handle, float *ms, int *kind, int capacity, int *count);
+int tnlm_profile_kernels(tnlm_handle *handle, int enable);
+int tnlm_kernel_times(tnlm_handle *handle, float *ms, int *kind, int capacity, int *count);
 
 /* Measured FP32 (non-tensor) FMA peak of the current device in TFLOP/s (2 flops per FFMA): an
  * 8-chain FFMA kernel on every SM, best of 3 timed launches on `stream` (synchronises).  The
@@ -158,7 +187,7 @@ int tnlm_fma_peak(double *tflops, void *stream);
 /* Number of CUDA kernels this handle has launched so far (for benchmark bookkeeping). */
 long long tnlm_launch_count(const tnlm_handle *handle);
 
-/* Library version string, e.g. "tnlm-b200 0.1 (sm_100a)". */
+/* Library version string, e.g. "tnlm-b200 0.2 (sm_100a)". */
 const char *tnlm_version(void);
 
 #ifdef __cplusplus

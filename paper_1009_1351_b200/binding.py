@@ -14,9 +14,12 @@ STATUS = {0: "TNLM_OK", 1: "TNLM_INVALID_ARG", 2: "TNLM_CUDA_ERROR", 3: "TNLM_AL
 EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "tnlm_cgls_step",
            "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
            "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version",
-           "tnlm_profile_sweeps", "tnlm_sweep_times", "tnlm_fbp_init", "tnlm_fma_peak"]
+           "tnlm_profile_kernels", "tnlm_kernel_times", "tnlm_fbp_init", "tnlm_fma_peak",
+           "tnlm_reserve", "tnlm_set_option", "tnlm_device"]
 
-KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply"}
+# tnlm_kernel_kind
+KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply", 3: "project", 4: "backproject", 5: "transpose",
+                6: "cgls_vector", 7: "clip", 8: "fbp"}
 
 
 class TnlmError(RuntimeError):
@@ -73,10 +76,13 @@ def library():
         L.tnlm_launch_count.argtypes = [P]
         L.tnlm_launch_count.restype = C.c_longlong
         L.tnlm_version.restype = C.c_char_p
-        L.tnlm_profile_sweeps.argtypes = [P, I]
+        L.tnlm_profile_kernels.argtypes = [P, I]
         L.tnlm_fbp_init.argtypes = [P, P, P, I, P]
         L.tnlm_fma_peak.argtypes = [C.POINTER(C.c_double), P]
-        L.tnlm_sweep_times.argtypes = [P, C.POINTER(C.c_float), C.POINTER(I), I, C.POINTER(I)]
+        L.tnlm_kernel_times.argtypes = [P, C.POINTER(C.c_float), C.POINTER(I), I, C.POINTER(I)]
+        L.tnlm_reserve.argtypes = [P, I, I, I, I]
+        L.tnlm_set_option.argtypes = [P, C.c_char_p, C.c_longlong]
+        L.tnlm_device.argtypes = [P]
         _LIB = L
     return _LIB
 
@@ -90,6 +96,13 @@ class Handle:
 
     def __init__(self, ptr, nx, ny, n_phase, geometry):
         self.ptr, self.nx, self.ny, self.n_phase, self.geometry = ptr, nx, ny, n_phase, geometry
+        self.device = int(library().tnlm_device(ptr))          # the CUDA device the handle lives on
+        self.img_per_slice = n_phase * ny * nx
+        self.sino_per_slice = n_phase * geometry.n_views * geometry.n_bins if geometry is not None else 0
+
+    def sino_count(self, n_slices):
+        """Elements of a sinogram argument for n_slices (None without geometry: the library reports that)."""
+        return n_slices * self.sino_per_slice if self.geometry is not None else None
 
     def close(self):
         if self.ptr:
@@ -131,12 +144,18 @@ def create(geometry, nx, ny, n_phase, window, patch, h, mu) -> Handle:
 
 
 # ---- device-pointer calls: torch tensors provide memory and the current stream -----------------
-def _dev(t, name):
+# Every tensor argument is checked here (dtype, contiguity, device of the handle, element count
+# for the number of slices the call names): the C side sees raw pointers and cannot.
+def _dev(h, t, name, count=None):
     import torch
     if t is None:
         return None
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
         raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+    if t.device.index != h.device:
+        raise ValueError(f"{name} is on cuda:{t.device.index}, the handle was created on cuda:{h.device}")
+    if count is not None and t.numel() != count:
+        raise ValueError(f"{name} has {t.numel()} elements, the call needs {count}")
     return t.data_ptr()
 
 
@@ -145,49 +164,65 @@ def _stream(stream):
     return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
 
 
-def _slices(h: Handle, t, per_slice):
+def _slices(t, per_slice, name):
     n = t.numel()
-    if n % per_slice:
-        raise ValueError("tensor size is not a whole number of slices")
+    if per_slice <= 0 or n == 0 or n % per_slice:
+        raise ValueError(f"{name}: size is not a whole number of slices")
     return n // per_slice
 
 
 def project(h: Handle, img, sino, stream=None):
-    S = _slices(h, img, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_project(h.ptr, _dev(img, "img"), _dev(sino, "sino"), S, _stream(stream)))
+    S = _slices(img, h.img_per_slice, "img")
+    h.check(library().tnlm_project(h.ptr, _dev(h, img, "img"), _dev(h, sino, "sino", h.sino_count(S)), S,
+                                   _stream(stream)))
     return sino
 
 
 def backproject(h: Handle, sino, img, stream=None):
-    S = _slices(h, img, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_backproject(h.ptr, _dev(sino, "sino"), _dev(img, "img"), S, _stream(stream)))
+    S = _slices(img, h.img_per_slice, "img")
+    h.check(library().tnlm_backproject(h.ptr, _dev(h, sino, "sino", h.sino_count(S)), _dev(h, img, "img"), S,
+                                       _stream(stream)))
     return img
 
 
 def fbp_init(h: Handle, y, f0, stream=None):
-    S = _slices(h, f0, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_fbp_init(h.ptr, _dev(y, "y"), _dev(f0, "f0"), S, _stream(stream)))
+    S = _slices(f0, h.img_per_slice, "f0")
+    h.check(library().tnlm_fbp_init(h.ptr, _dev(h, y, "y", h.sino_count(S)), _dev(h, f0, "f0"), S, _stream(stream)))
     return f0
 
 
 def cgls_step(h: Handle, f_in, y, w, m1, g_out, stream=None):
-    S = _slices(h, f_in, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_cgls_step(h.ptr, _dev(f_in, "f_in"), _dev(y, "y"), _dev(w, "w"), m1,
-                                     _dev(g_out, "g_out"), S, _stream(stream)))
+    S = _slices(f_in, h.img_per_slice, "f_in")
+    ns = h.sino_count(S)
+    h.check(library().tnlm_cgls_step(h.ptr, _dev(h, f_in, "f_in"), _dev(h, y, "y", ns), _dev(h, w, "w", ns), m1,
+                                     _dev(h, g_out, "g_out", S * h.img_per_slice), S, _stream(stream)))
     return g_out
 
 
 def regularize_step(h: Handle, g, m2, f_out, stream=None):
-    S = _slices(h, g, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_regularize_step(h.ptr, _dev(g, "g"), m2, _dev(f_out, "f_out"), S, _stream(stream)))
+    S = _slices(g, h.img_per_slice, "g")
+    h.check(library().tnlm_regularize_step(h.ptr, _dev(h, g, "g"), m2, _dev(h, f_out, "f_out", S * h.img_per_slice), S,
+                                           _stream(stream)))
     return f_out
 
 
 def reconstruct(h: Handle, y, w, f0, k_outer, m1, m2, f_out, stream=None):
-    S = _slices(h, f_out, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_reconstruct(h.ptr, _dev(y, "y"), _dev(w, "w"), _dev(f0, "f0"), k_outer, m1, m2,
-                                       _dev(f_out, "f_out"), S, _stream(stream)))
+    S = _slices(f_out, h.img_per_slice, "f_out")
+    ns = h.sino_count(S)
+    h.check(library().tnlm_reconstruct(h.ptr, _dev(h, y, "y", ns), _dev(h, w, "w", ns),
+                                       _dev(h, f0, "f0", S * h.img_per_slice), k_outer, m1, m2,
+                                       _dev(h, f_out, "f_out"), S, _stream(stream)))
     return f_out
+
+
+def reserve(h: Handle, n_slices, m1, m2, host_entry_points=False):
+    """tnlm_reserve: allocate the workspace now so that later enqueue calls never allocate."""
+    h.check(library().tnlm_reserve(h.ptr, n_slices, m1, m2, int(bool(host_entry_points))))
+
+
+def set_option(h: Handle, name: str, value: int):
+    """tnlm_set_option: "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns"."""
+    h.check(library().tnlm_set_option(h.ptr, name.encode(), int(value)))
 
 
 def fma_peak(stream=None) -> float:
@@ -199,39 +234,43 @@ def fma_peak(stream=None) -> float:
     return float(out.value)
 
 
-def profile_sweeps(h: Handle, enable: bool):
-    h.check(library().tnlm_profile_sweeps(h.ptr, int(bool(enable))))
+def profile_kernels(h: Handle, enable: bool):
+    h.check(library().tnlm_profile_kernels(h.ptr, int(bool(enable))))
 
 
-def sweep_times(h: Handle, capacity: int = 4096):
-    """[(kind name, milliseconds)] of the TNLM kernel launches recorded since the last call."""
+def kernel_times(h: Handle, capacity: int = 16384):
+    """[(kind name, milliseconds)] of the kernel launches recorded since the last call."""
     ms = (C.c_float * capacity)()
     kind = (C.c_int * capacity)()
     n = C.c_int(0)
-    h.check(library().tnlm_sweep_times(h.ptr, ms, kind, capacity, C.byref(n)))
+    h.check(library().tnlm_kernel_times(h.ptr, ms, kind, capacity, C.byref(n)))
     return [(KERNEL_KINDS.get(kind[i], str(kind[i])), float(ms[i])) for i in range(min(n.value, capacity))]
 
 
 # ---- host-pointer calls: CPU tensors (pinned or pageable); copies happen inside the library ----
-def _host(t, name):
+def _host(t, name, count=None):
     import torch
     if t is None:
         return None
     if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
         raise TypeError(f"{name} must be a contiguous float32 CPU tensor")
+    if count is not None and t.numel() != count:
+        raise ValueError(f"{name} has {t.numel()} elements, the call needs {count}")
     return t.data_ptr()
 
 
 def regularize_step_host(h: Handle, g_host, m2, f_out_host, stream=None):
-    S = _slices(h, g_host, h.n_phase * h.nx * h.ny)
+    S = _slices(g_host, h.img_per_slice, "g_host")
     h.check(library().tnlm_regularize_step_host(h.ptr, _host(g_host, "g_host"), m2,
-                                                _host(f_out_host, "f_out_host"), S, _stream(stream)))
+                                                _host(f_out_host, "f_out_host", S * h.img_per_slice), S,
+                                                _stream(stream)))
     return f_out_host
 
 
 def reconstruct_host(h: Handle, y_host, w_host, f0_host, k_outer, m1, m2, f_out_host, stream=None):
-    S = _slices(h, f_out_host, h.n_phase * h.nx * h.ny)
-    h.check(library().tnlm_reconstruct_host(h.ptr, _host(y_host, "y_host"), _host(w_host, "w_host"),
-                                            _host(f0_host, "f0_host"), k_outer, m1, m2,
+    S = _slices(f_out_host, h.img_per_slice, "f_out_host")
+    ns = h.sino_count(S)
+    h.check(library().tnlm_reconstruct_host(h.ptr, _host(y_host, "y_host", ns), _host(w_host, "w_host", ns),
+                                            _host(f0_host, "f0_host", S * h.img_per_slice), k_outer, m1, m2,
                                             _host(f_out_host, "f_out_host"), S, _stream(stream)))
     return f_out_host

@@ -2,6 +2,13 @@
 // (gamma_m = ||P_n^T r^(m)||^2, qq_m = ||P_n s^(m)||^2) live on the device as doubles, one per
 // (slice, phase) problem and inner step; kernels derive a_m and b_m from them on the fly, so
 // nothing synchronises with the host.
+//
+// Launches per inner step m (tnlm_api.cu, cgls_device):
+//   project_kernel<FWD_SCALE>   q = sqrt(w) P s_m, qq_m                      (reads s_m and its transpose)
+//   cgls_update_r               r -= a_m q ; rw = sqrt(w) r                   (sinogram pass)
+//   backproject_kernel          t = P^T rw, gamma_{m+1}
+//   cgls_update_us              u += a_m s_m ; s_{m+1} = t + b_m s_m ; sT = s_{m+1}^T   (one image pass)
+// The last step only needs u += a_m s_m (cgls_update_us<true>): r, t, s of step M1 feed nothing (L127).
 #pragma once
 #include "common.cuh"
 
@@ -26,45 +33,74 @@ __device__ __forceinline__ float cgls_b(const double *gam, const double *qq, int
     return (float)(gam[(size_t)(m + 1) * nprob + prob] / gam[(size_t)m * nprob + prob]); // step 4 (L125)
 }
 
-// u += a s (step 2, L114);  grid = (ceil(npix/256), nprob)
-__global__ void cgls_update_u(float *__restrict__ u, const float *__restrict__ s, int npix,
-                              const double *gam, const double *qq, int nprob, int m)
+// sw = sqrt(w): the diagonal of Sigma^-1/2 (L103), computed once per call instead of once per use.
+__global__ void sqrt_weights_kernel(const float *__restrict__ w, float *__restrict__ sw, size_t n)
 {
-    const int prob = blockIdx.y;
-    const float a = cgls_a(gam, qq, nprob, prob, m);
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < npix) {
-        const size_t o = (size_t)prob * npix + i;
-        u[o] = fmaf(a, s[o], u[o]);
-    }
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) sw[i] = sqrtf(w[i]);
 }
 
 // r -= a q (step 3, L115);  rw = sqrt(w) r (the sinogram P_n^T gathers);  grid = (ceil(nray/256), nprob)
-__global__ void cgls_update_r(float *__restrict__ r, float *__restrict__ rw, const float *__restrict__ q,
-                              const float *__restrict__ w, int nray, const double *gam,
-                              const double *qq, int nprob, int m)
+__global__ void __launch_bounds__(256)
+cgls_update_r(float *__restrict__ r, float *__restrict__ rw, const float *__restrict__ q,
+              const float *__restrict__ sw, int nray, const double *gam, const double *qq, int nprob, int m)
 {
+    __shared__ float a_sh;
     const int prob = blockIdx.y;
-    const float a = cgls_a(gam, qq, nprob, prob, m);
+    if (threadIdx.x == 0) a_sh = cgls_a(gam, qq, nprob, prob, m);
+    __syncthreads();
+    const float a = a_sh;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < nray) {
         const size_t o = (size_t)prob * nray + i;
         const float rn = fmaf(-a, q[o], r[o]);
         r[o] = rn;
-        rw[o] = (w ? sqrtf(w[o]) : 1.0f) * rn;
+        rw[o] = (sw ? sw[o] : 1.0f) * rn;
     }
 }
 
-// s = t + b s (step 5, L126);  a broken-down phase keeps s (it is never used again)
-__global__ void cgls_update_s(float *__restrict__ s, const float *__restrict__ t, int npix,
-                              const double *gam, const double *qq, int nprob, int m)
+// u += a_m s (step 2, L114) and, unless LAST, s = t + b_m s (step 5, L126) with the transposed copy sT
+// the forward projector reads for its shallow rays, in one pass over 32 x 32 image tiles.
+// A broken-down phase has a = b = 0: u stays, s = t (never used again).
+// grid = (ceil(nx/32), ceil(ny/32), nprob); block = (32, 8).
+template <bool LAST>
+__global__ void __launch_bounds__(256)
+cgls_update_us(float *__restrict__ u, float *__restrict__ s, const float *__restrict__ t, float *__restrict__ sT,
+               int nx, int ny, const double *gam, const double *qq, int nprob, int m)
 {
-    const int prob = blockIdx.y;
-    const float b = cgls_b(gam, qq, nprob, prob, m);
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < npix) {
-        const size_t o = (size_t)prob * npix + i;
-        s[o] = fmaf(b, s[o], t[o]);
+    __shared__ float tile[32][33];
+    __shared__ float ab[2];
+    const int prob = blockIdx.z;
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+        ab[0] = cgls_a(gam, qq, nprob, prob, m);
+        ab[1] = LAST ? 0.f : cgls_b(gam, qq, nprob, prob, m);
+    }
+    __syncthreads();
+    const float a = ab[0], b = ab[1];
+    const size_t base = (size_t)prob * nx * ny;
+    const int c = blockIdx.x * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int r = blockIdx.y * 32 + threadIdx.y + j;
+        float sn = 0.f;
+        if (r < ny && c < nx) {
+            const size_t o = base + (size_t)r * nx + c;
+            const float so = s[o];
+            u[o] = fmaf(a, so, u[o]);
+            if (!LAST) {
+                sn = fmaf(b, so, t[o]);
+                s[o] = sn;
+            }
+        }
+        if (!LAST) tile[threadIdx.y + j][threadIdx.x] = sn;
+    }
+    if (LAST) return;
+    __syncthreads();
+    const int rT = blockIdx.y * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int cT = blockIdx.x * 32 + threadIdx.y + j;
+        if (rT < ny && cT < nx) sT[base + (size_t)cT * ny + rT] = tile[threadIdx.x][threadIdx.y + j];
     }
 }
 

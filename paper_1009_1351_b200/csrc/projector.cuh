@@ -11,6 +11,7 @@ enum FwdMode {
     FWD_PLAIN = 0,  // out0 = P img
     FWD_RESID = 1,  // out0 = sw*(y - P img) = r ; out1 = sw*r            (CGLS init, L109)
     FWD_SCALE = 2   // out0 = sw*(P img) = q ; red += ||q||^2             (CGLS step 1, L112)
+                    // sw = sqrt(w), the diagonal of Sigma^-1/2 (L103), precomputed (NULL = 1)
 };
 
 // atan on the fan-angle range: odd minimax polynomial on [-1, 1] (Abramowitz & Stegun 4.4.49,
@@ -61,7 +62,7 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
                const float *__restrict__ img, const float *__restrict__ imgT, const float *__restrict__ y,
-               const float *__restrict__ w, float *__restrict__ out0, float *__restrict__ out1,
+               const float *__restrict__ sw_, float *__restrict__ out0, float *__restrict__ out1,
                double *__restrict__ red)
 {
     const int prob = blockIdx.y;                 // slice*N + phase
@@ -108,7 +109,7 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
         if (MODE == FWD_PLAIN) {
             out0[o] = p;
         } else {
-            const float sw = w ? sqrtf(w[o]) : 1.0f;
+            const float sw = sw_ ? sw_[o] : 1.0f;
             if (MODE == FWD_RESID) {
                 const float r = sw * (y[o] - p);
                 out0[o] = r;

@@ -16,12 +16,14 @@
 // Per weight evaluation this costs 2 FSUB-slots + 2.75 FMA (box rows, x 1+2b/RB for the warm-up
 // rows) + 2 FADD (vertical) + 4: about 12 FP32 instructions against 2d+4 = 14 algorithmic flops.
 //
-// Softmax reference.  w = exp(-D/h^2)/Z is evaluated as 2^(c*(D0(x) - D(x,delta)) - 90),
+// Softmax reference.  w = exp(-D/h^2)/Z is evaluated as 2^(c*(D0(x) - D(x,delta)) - 100),
 // c = log2(e)/h^2, D0 = the distance at delta = 0 (always a valid candidate), so the delta = 0
-// term is 2^-90 and Z can never underflow to 0; a candidate more than 217/c better than
-// delta = 0 overflows to +inf, which flags the pixel, and flagged pixels are recomputed by the
-// warp with the minimum-subtracted two-pass form (exact_side_ratio) straight from the shared
-// tiles.  The value is always the softmax of Eq. (3); the reference only picks the fp32 range.
+// term is 2^-100 and Z can never underflow to 0; a pixel whose weight sum reaches 2^100 (a candidate
+// about 200/c better than delta = 0) or whose numerator is not below 2^120 is flagged, and flagged
+// pixels are recomputed by the warp with the minimum-subtracted two-pass form (exact_side_ratio)
+// straight from the shared tiles.  With Z < 2^100 the numerator sum_delta e u_j stays finite for
+// |u| < 2^17 (documented in tnlm.h), here and in gj_apply_kernel, which re-reads the same weights.
+// The value is always the softmax of Eq. (3); the reference only picks the fp32 range.
 //
 // Borders.  Tiles are zero-filled outside the image (patches are zero-extended, DESIGN.md
 // reading 7).  A candidate column outside the image (or a dc beyond the window in the last
@@ -35,7 +37,7 @@
 // wts[image][side][band][tile_x][delta][RB rows][128 columns] -- one contiguous chunk per warp
 // band, written and later read as a sequential stream (DRAM-page friendly; a plane-per-offset
 // layout scatters 256-byte pieces and ran 3x slower).  bf16 keeps the fp32 exponent range, so the
-// stored values are the very 2^(c(D0-D)-90) of the fast path (an fp16 version needed its own
+// stored values are the very 2^(c(D0-D)-100) of the fast path (an fp16 version needed its own
 // reference and sent every moving edge through the slow exact route: 2.6x slower); the quotient
 // A/Z of Eq. (7) does not depend on the per-pixel scale, and the 2^-9 rounding of each weight
 // moves it by < 1e-6 relative.  Pixels on the exact route store their
@@ -72,8 +74,9 @@ struct SweepParams {
     float c_self;           // 1/(1+mu)
     float c_nb;             // mu/(2mu+2)
     float big_d;            // distance given to excluded candidates (finite, big_d*pos_c finite)
-    float margin;           // the delta = 0 weight is 2^-margin (90)
-    float z_limit;          // a side whose weight sum is not below this is recomputed exactly
+    float margin;           // the delta = 0 weight is 2^-margin (100)
+    float z_limit;          // a side whose weight sum is not below this (2^100) is recomputed exactly
+    float a_limit;          // ... or whose numerator magnitude is not below this (2^120)
     int clip;               // apply max(.,0) to the output
     int ap_ns;              // gj_apply_kernel: stages of its bulk-copy ring
 };
@@ -225,7 +228,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     const float *__restrict__ myUj = sUj + side * uj_rows * UJW;
     float *__restrict__ myK = sK + warp * RB * SW_TW;
 
-    // ---- reference exponents K(x) = c*D0(x) - 90, D0 = distance at delta = 0 (same march, one offset)
+    // ---- reference exponents K(x) = c*D0(x) - margin, D0 = distance at delta = 0 (same march, one offset)
     {
         float D0[C], ring[C][RING];
 #pragma unroll
@@ -386,7 +389,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             const bool valid = (r0 + rr < ny) && (c0 + c < nx);
             float &Arc = (c & 1) ? A[rr][c >> 1].y : A[rr][c >> 1].x;
             const float Zrc = (c & 1) ? Z[rr][c >> 1].y : Z[rr][c >> 1].x;
-            const bool bad = valid && !(Zrc < p.z_limit);
+            const bool bad = valid && (!(Zrc < p.z_limit) || !(fabsf(Arc) < p.a_limit));
             Arc = Arc / Zrc;
             unsigned m = __ballot_sync(0xffffffffu, bad);
             while (m) {

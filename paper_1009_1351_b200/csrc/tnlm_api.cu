@@ -10,6 +10,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "../../include/tnlm.h"
 #include "cgls.cuh"
 #include "common.cuh"
@@ -37,8 +39,12 @@ struct tnlm_handle {
     Geom G{};
     SweepParams R{};
     std::vector<SweepShape> shapes;   // launchable sweep shapes for this (window, patch)
+    int device = 0;         // the CUDA device the handle was created on; every entry point runs there
     int n_sm = 148;
     size_t smem_per_sm = 233472;
+    // tuning knobs, read once from the environment at tnlm_create (tnlm_set_option changes them later)
+    long long opt_cache_mb = 16384;
+    int opt_rb = 0, opt_nb = 0, opt_ns = 0;
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
@@ -52,7 +58,7 @@ struct tnlm_handle {
     float *d_s = nullptr, *d_t = nullptr, *d_g = nullptr, *d_f = nullptr;  // images
     float *d_ua = nullptr, *d_ub = nullptr;                                  // sweep ping-pong
     float *d_imT = nullptr;                                                  // transposed image of the forward projector
-    float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr;                   // sinograms
+    float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr, *d_sw = nullptr;  // sinograms (d_sw = sqrt(w))
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
     __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
     size_t wts_cap = 0;               // in halves
@@ -67,7 +73,29 @@ struct tnlm_handle {
     std::string err;
 };
 
-static std::string g_create_error;
+static thread_local std::string g_create_error;     // message of the last failed tnlm_create of this thread
+
+// NVTX range around a C-ABI call (visible in nsys / ncu --nvtx; free when no tool is attached).
+struct NvtxRange {
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+
+// Makes the handle's device current for the duration of a call and restores the caller's.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev)
+    {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) {
+            err = cudaSetDevice(dev);
+            switched = (err == cudaSuccess);
+        }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 static int fail(tnlm_handle *h, int code, const std::string &msg)
 {
@@ -90,7 +118,7 @@ static int cuda_fail(tnlm_handle *h, cudaError_t e, const char *what)
         if (e__ != cudaSuccess) return cuda_fail(h, e__, "kernel launch"); \
     } while (0)
 
-extern "C" const char *tnlm_version(void) { return "tnlm-b200 0.1 (sm_100a)"; }
+extern "C" const char *tnlm_version(void) { return "tnlm-b200 0.2 (sm_100a)"; }
 
 extern "C" const char *tnlm_last_error(const tnlm_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
@@ -167,19 +195,19 @@ static cudaError_t add_sweep_shapes(tnlm_handle *H, size_t smem_limit)
 {
     const void *fn = (const void *)gj_sweep_kernel<PB, RB, false>;
     const void *fn_store = (const void *)gj_sweep_kernel<PB, RB, true>;
-    size_t biggest = 0;
     std::vector<SweepShape> mine;
     for (int nb = 4; nb >= 1; nb >>= 1) {
         SweepShape sh;
         sh.fn = fn; sh.fn_store = fn_store; sh.rb = RB; sh.nb = nb;
         sh.smem = SweepGeom<PB>::smem_words(H->R.a, H->R.ngroups, nb, RB) * sizeof(float);
         if (sh.smem > smem_limit) continue;
-        if (sh.smem > biggest) biggest = sh.smem;
         mine.push_back(sh);
     }
     if (mine.empty()) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)biggest);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_store, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)biggest);
+    // The attribute belongs to the kernel symbol, not to the handle: always the device maximum, so that a
+    // later handle with a smaller window can never lower it under a live handle's launches.
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_limit);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fn_store, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_limit);
     if (e != cudaSuccess) return e;
     for (SweepShape &sh : mine) {
         int occ_store = 0;
@@ -231,6 +259,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     if (window < 1 || patch < 1 || (window & 1) == 0 || (patch & 1) == 0)
         return fail(nullptr, TNLM_INVALID_ARG, "window and patch must be odd and >= 1");
     if (!(h > 0.f) || !std::isfinite(h)) return fail(nullptr, TNLM_INVALID_ARG, "h must be finite and > 0");
+    if (h > 1e12f) return fail(nullptr, TNLM_INVALID_ARG, "h above 1e12: excluded candidates could no longer be given weight 0");
     if (!(mu >= 0.f) || !std::isfinite(mu)) return fail(nullptr, TNLM_INVALID_ARG, "mu must be finite and >= 0");
     if (patch > MAX_PATCH || window > MAX_WINDOW)
         return fail(nullptr, TNLM_UNSUPPORTED, "patch > 9 or window > 31 not compiled");
@@ -254,6 +283,10 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     tnlm_handle *H = new (std::nothrow) tnlm_handle();
     if (!H) return fail(nullptr, TNLM_ALLOC_FAILED, "host allocation failed");
     H->nx = nx; H->ny = ny; H->n_phase = n_phase; H->window = window; H->patch = patch; H->h = h; H->mu = mu;
+    H->device = dev;
+    if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) H->opt_cache_mb = std::strtoll(ev, nullptr, 10);
+    if (const char *ev = std::getenv("TNLM_SWEEP_SHAPE")) std::sscanf(ev, "%d,%d", &H->opt_rb, &H->opt_nb);
+    if (const char *ev = std::getenv("TNLM_APPLY_NS")) H->opt_ns = std::atoi(ev);
 
     // TNLM parameters
     SweepParams &R = H->R;
@@ -265,11 +298,12 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     R.c_self = (float)(1.0 / (1.0 + (double)mu));
     R.c_nb = (float)((double)mu / (2.0 * (double)mu + 2.0));
     R.big_d = (float)std::fmin(1e30, 1e37 / c);
-    R.margin = 90.0f;
-    R.z_limit = 1.0e38f;
+    R.margin = 100.0f;
+    R.z_limit = 1.2676506e30f;      // 2^100
+    R.a_limit = 1.3292280e36f;      // 2^120
     R.clip = 0;
     {
-        H->apply_smem = std::min(apply_smem_bytes(window, 10, AP_NS_MAX), (size_t)prop.sharedMemPerBlockOptin);   // rb <= 10
+        H->apply_smem = (size_t)prop.sharedMemPerBlockOptin;     // per kernel symbol: always the device maximum
         ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)H->apply_smem);
         // ask for the largest shared-memory carveout so that the ring-depth choice below decides the occupancy
@@ -355,7 +389,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
 
 static void free_ws(tnlm_handle *H)
 {
-    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_fbp_q, &H->d_r, &H->d_rw, &H->d_q, &H->d_yh, &H->d_wh};
+    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_fbp_q, &H->d_r, &H->d_rw, &H->d_q, &H->d_sw, &H->d_yh, &H->d_wh};
     for (float **b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     H->ws_slices = 0;
 }
@@ -363,6 +397,7 @@ static void free_ws(tnlm_handle *H)
 extern "C" int tnlm_destroy(tnlm_handle *H)
 {
     if (!H) return TNLM_INVALID_ARG;
+    DeviceGuard dg(H->device);
     for (cudaEvent_t e : H->prof_ev) cudaEventDestroy(e);
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
@@ -377,7 +412,8 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     return TNLM_OK;
 }
 
-// Workspace for n_slices (grown, never shrunk).  Buffers are allocated on first need of their kind.
+// Workspace for n_slices (grown, never shrunk).  Buffers are allocated on first need of their kind
+// (cudaMalloc synchronises the device: see "Execution" in tnlm.h; tnlm_reserve front-loads it).
 static int ensure_ws(tnlm_handle *H, int n_slices)
 {
     if (n_slices <= H->ws_slices) return TNLM_OK;
@@ -404,25 +440,71 @@ static int check_common(tnlm_handle *H, int n_slices, bool needs_geom)
     if (needs_geom && !H->has_geom) return fail(H, TNLM_INVALID_ARG, "handle was created without geometry");
     return TNLM_OK;
 }
+#define ENTER(H, name, n_slices, needs_geom)                                   \
+    NvtxRange nvtx_range__(name);                                              \
+    {                                                                          \
+        int rc__ = check_common(H, n_slices, needs_geom);                      \
+        if (rc__) return rc__;                                                 \
+    }                                                                          \
+    DeviceGuard device_guard__((H)->device);                                   \
+    if (device_guard__.err != cudaSuccess) return cuda_fail(H, device_guard__.err, "cudaSetDevice")
+
+// ------------------------------------------------------------------------------ per-launch timing
+// Event pair around one kernel launch, on the launching stream (tnlm_profile_kernels).
+static int prof_mark(tnlm_handle *H, int kind, bool begin, cudaStream_t st)
+{
+    if (begin) {
+        const size_t need = 2 * H->prof_kind.size() + 2;
+        while (H->prof_ev.size() < need) {
+            cudaEvent_t e;
+            CU(H, cudaEventCreate(&e));
+            H->prof_ev.push_back(e);
+        }
+        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size()], st));
+        H->prof_kind.push_back(kind);
+    } else {
+        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size() - 1], st));
+    }
+    return TNLM_OK;
+}
+struct ProfScope {
+    tnlm_handle *H;
+    cudaStream_t st;
+    bool on;
+    ProfScope(tnlm_handle *h, int kind, cudaStream_t s) : H(h), st(s), on(h->prof) { if (on) prof_mark(H, kind, true, st); }
+    ~ProfScope() { if (on) prof_mark(H, 0, false, st); }
+};
 
 // ------------------------------------------------------------------------------ projector
+static int launch_transpose(tnlm_handle *H, const float *img, float *imgT, int n_slices, cudaStream_t st)
+{
+    ProfScope ps(H, TNLM_KERNEL_TRANSPOSE, st);
+    dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, n_slices * H->n_phase);
+    transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(img, imgT, H->nx, H->ny);
+    LAUNCHED(H);
+    return TNLM_OK;
+}
+// imgT = the transposed copy of img the shallow rays walk; NULL = make it here (d_imT).
 template <int MODE>
-static int launch_project(tnlm_handle *H, const float *img, const float *y, const float *w, float *out0,
-                          float *out1, double *red, int n_slices, cudaStream_t st)
+static int launch_project(tnlm_handle *H, const float *img, const float *imgT, const float *y, const float *sw,
+                          float *out0, float *out1, double *red, int n_slices, cudaStream_t st)
 {
     const int nray = H->G.n_views * H->G.n_bins;
-    int rc = need(H, &H->d_imT, img_count(H));
-    if (rc) return rc;
-    dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, n_slices * H->n_phase);
-    transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(img, H->d_imT, H->nx, H->ny);
-    LAUNCHED(H);
+    int rc;
+    if (!imgT) {
+        if ((rc = need(H, &H->d_imT, img_count(H)))) return rc;
+        if ((rc = launch_transpose(H, img, H->d_imT, n_slices, st))) return rc;
+        imgT = H->d_imT;
+    }
+    ProfScope ps(H, TNLM_KERNEL_PROJECT, st);
     dim3 grid((nray + 255) / 256, n_slices * H->n_phase);
-    project_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, H->d_imT, y, w, out0, out1, red);
+    project_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red);
     LAUNCHED(H);
     return TNLM_OK;
 }
 static int launch_backproject(tnlm_handle *H, const float *sino, float *img, double *red, int n_slices, cudaStream_t st)
 {
+    ProfScope ps(H, TNLM_KERNEL_BACKPROJECT, st);
     dim3 grid((H->nx + 15) / 16, (H->ny + 31) / 32, n_slices * H->n_phase);
     if (H->fan_poly) backproject_kernel<true><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
     else backproject_kernel<false><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
@@ -432,17 +514,16 @@ static int launch_backproject(tnlm_handle *H, const float *sino, float *img, dou
 
 extern "C" int tnlm_project(tnlm_handle *H, const float *img, float *sino, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_project", n_slices, true);
+    int rc;
     if (!img || !sino) return fail(H, TNLM_INVALID_ARG, "img and sino must not be NULL");
     if ((rc = ensure_ws(H, n_slices))) return rc;
-    return launch_project<FWD_PLAIN>(H, img, nullptr, nullptr, sino, nullptr, nullptr, n_slices, (cudaStream_t)stream);
+    return launch_project<FWD_PLAIN>(H, img, nullptr, nullptr, nullptr, sino, nullptr, nullptr, n_slices, (cudaStream_t)stream);
 }
 
 extern "C" int tnlm_backproject(tnlm_handle *H, const float *sino, float *img, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_backproject", n_slices, true);
     if (!img || !sino) return fail(H, TNLM_INVALID_ARG, "img and sino must not be NULL");
     return launch_backproject(H, sino, img, nullptr, n_slices, (cudaStream_t)stream);
 }
@@ -450,17 +531,21 @@ extern "C" int tnlm_backproject(tnlm_handle *H, const float *sino, float *img, i
 // ------------------------------------------------------------------------------ FBP initialisation
 extern "C" int tnlm_fbp_init(tnlm_handle *H, const float *y, float *f0, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_fbp_init", n_slices, true);
+    int rc;
     if (!y || !f0) return fail(H, TNLM_INVALID_ARG, "y and f0 must not be NULL");
     if ((size_t)H->G.n_bins * sizeof(float) > 48 * 1024) return fail(H, TNLM_UNSUPPORTED, "more than 12288 detector bins");
     if ((rc = ensure_ws(H, n_slices))) return rc;
     if ((rc = need(H, &H->d_fbp_q, sino_count(H)))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int M = H->n_phase * H->G.n_views;
-    fbp_filter_kernel<<<dim3(M, n_slices), 256, H->G.n_bins * sizeof(float), st>>>(y, H->d_fbp_q, H->d_fbp_cosw, H->d_fbp_g,
-                                                                                      H->G.n_bins);
-    LAUNCHED(H);
+    {
+        ProfScope ps(H, TNLM_KERNEL_FBP, st);
+        fbp_filter_kernel<<<dim3(M, n_slices), 256, H->G.n_bins * sizeof(float), st>>>(y, H->d_fbp_q, H->d_fbp_cosw, H->d_fbp_g,
+                                                                                          H->G.n_bins);
+        LAUNCHED(H);
+    }
+    ProfScope ps(H, TNLM_KERNEL_FBP, st);
     fbp_backproject_kernel<<<dim3((H->nx + 31) / 32, (H->ny + 7) / 8, n_slices), dim3(32, 8), 0, st>>>(
         H->G, H->d_views, H->d_fbp_wv, H->d_fbp_q, f0);
     LAUNCHED(H);
@@ -468,7 +553,43 @@ extern "C" int tnlm_fbp_init(tnlm_handle *H, const float *y, float *f0, int n_sl
 }
 
 // ------------------------------------------------------------------------------ CGLS
-static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const float *w, int m1, float *g_out,
+static int ensure_scalars(tnlm_handle *H, int nscal)
+{
+    if (nscal <= H->scal_cap) return TNLM_OK;
+    if (H->d_scal) cudaFree(H->d_scal);
+    H->d_scal = nullptr; H->scal_cap = 0;
+    if (cudaMalloc(&H->d_scal, (size_t)nscal * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(H, TNLM_ALLOC_FAILED, "device allocation failed (scalars)"); }
+    H->scal_cap = nscal;
+    return TNLM_OK;
+}
+static int cgls_workspace(tnlm_handle *H, int m1, int n_slices, bool weighted)
+{
+    int rc;
+    if (m1 == 0) return TNLM_OK;
+    if ((rc = need(H, &H->d_s, img_count(H)))) return rc;
+    if ((rc = need(H, &H->d_t, img_count(H)))) return rc;
+    if ((rc = need(H, &H->d_imT, img_count(H)))) return rc;
+    if ((rc = need(H, &H->d_r, sino_count(H)))) return rc;
+    if ((rc = need(H, &H->d_rw, sino_count(H)))) return rc;
+    if ((rc = need(H, &H->d_q, sino_count(H)))) return rc;
+    if (weighted && (rc = need(H, &H->d_sw, sino_count(H)))) return rc;
+    return ensure_scalars(H, (2 * m1 + 1) * n_slices * H->n_phase);
+}
+// sw = sqrt(w) into the handle's buffer (once per call; w is fixed across the outer iterations).
+static int prepare_sqrt_weights(tnlm_handle *H, const float *w, int n_slices, cudaStream_t st)
+{
+    if (!w) return TNLM_OK;
+    int rc;
+    if ((rc = need(H, &H->d_sw, sino_count(H)))) return rc;
+    const size_t n = (size_t)n_slices * H->n_phase * H->G.n_views * H->G.n_bins;
+    ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
+    sqrt_weights_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w, H->d_sw, n);
+    LAUNCHED(H);
+    return TNLM_OK;
+}
+
+// sw = sqrt(w) (NULL = identity), already prepared by the caller.
+static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const float *sw, int m1, float *g_out,
                        int n_slices, cudaStream_t st)
 {
     const int nprob = n_slices * H->n_phase;
@@ -477,36 +598,37 @@ static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const 
     if (g_out != f_in) CU(H, cudaMemcpyAsync(g_out, f_in, nimg * sizeof(float), cudaMemcpyDeviceToDevice, st));
     if (m1 == 0) return TNLM_OK;
     int rc;
-    if ((rc = need(H, &H->d_s, img_count(H)))) return rc;
-    if ((rc = need(H, &H->d_t, img_count(H)))) return rc;
-    if ((rc = need(H, &H->d_r, sino_count(H)))) return rc;
-    if ((rc = need(H, &H->d_rw, sino_count(H)))) return rc;
-    if ((rc = need(H, &H->d_q, sino_count(H)))) return rc;
+    if ((rc = cgls_workspace(H, m1, n_slices, sw != nullptr))) return rc;
     const int nscal = (2 * m1 + 1) * nprob;
-    if (nscal > H->scal_cap) {
-        if (H->d_scal) cudaFree(H->d_scal);
-        H->d_scal = nullptr; H->scal_cap = 0;
-        if (cudaMalloc(&H->d_scal, (size_t)nscal * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(H, TNLM_ALLOC_FAILED, "device allocation failed (scalars)"); }
-        H->scal_cap = nscal;
-    }
     double *gam = H->d_scal, *qq = H->d_scal + (size_t)(m1 + 1) * nprob;
     CU(H, cudaMemsetAsync(H->d_scal, 0, (size_t)nscal * sizeof(double), st));
     float *u = g_out;
-    dim3 gi((npix + 255) / 256, nprob), gs((nray + 255) / 256, nprob);
+    dim3 gs((nray + 255) / 256, nprob), gt((H->nx + 31) / 32, (H->ny + 31) / 32, nprob);
     // init (L109): r = y_n - P_n u ; s = P_n^T r ; gamma_0 = ||s||^2
-    if ((rc = launch_project<FWD_RESID>(H, u, y, w, H->d_r, H->d_rw, nullptr, n_slices, st))) return rc;
+    if ((rc = launch_project<FWD_RESID>(H, u, nullptr, y, sw, H->d_r, H->d_rw, nullptr, n_slices, st))) return rc;
     if ((rc = launch_backproject(H, H->d_rw, H->d_s, gam, n_slices, st))) return rc;
+    const float *sT = nullptr;                       // transposed s: made by cgls_update_us from step 1 on
     for (int m = 0; m < m1; ++m) {
         // q = P_n s ; qq_m = ||q||^2
-        if ((rc = launch_project<FWD_SCALE>(H, H->d_s, nullptr, w, H->d_q, nullptr, qq + (size_t)m * nprob, n_slices, st))) return rc;
-        cgls_update_u<<<gi, 256, 0, st>>>(u, H->d_s, npix, gam, qq, nprob, m);
-        LAUNCHED(H);
-        if (m + 1 == m1) break;      // r, t, s of the last step feed nothing (g = u^(M1), L127)
-        cgls_update_r<<<gs, 256, 0, st>>>(H->d_r, H->d_rw, H->d_q, w, nray, gam, qq, nprob, m);
-        LAUNCHED(H);
+        if ((rc = launch_project<FWD_SCALE>(H, H->d_s, sT, nullptr, sw, H->d_q, nullptr, qq + (size_t)m * nprob, n_slices, st))) return rc;
+        if (m + 1 == m1) {                           // r, t, s of the last step feed nothing (g = u^(M1), L127)
+            ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
+            cgls_update_us<true><<<gt, dim3(32, 8), 0, st>>>(u, H->d_s, nullptr, nullptr, H->nx, H->ny, gam, qq, nprob, m);
+            LAUNCHED(H);
+            break;
+        }
+        {
+            ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
+            cgls_update_r<<<gs, 256, 0, st>>>(H->d_r, H->d_rw, H->d_q, sw, nray, gam, qq, nprob, m);
+            LAUNCHED(H);
+        }
         if ((rc = launch_backproject(H, H->d_rw, H->d_t, gam + (size_t)(m + 1) * nprob, n_slices, st))) return rc;
-        cgls_update_s<<<gi, 256, 0, st>>>(H->d_s, H->d_t, npix, gam, qq, nprob, m);
-        LAUNCHED(H);
+        {
+            ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
+            cgls_update_us<false><<<gt, dim3(32, 8), 0, st>>>(u, H->d_s, H->d_t, H->d_imT, H->nx, H->ny, gam, qq, nprob, m);
+            LAUNCHED(H);
+        }
+        sT = H->d_imT;
     }
     return TNLM_OK;
 }
@@ -514,12 +636,14 @@ static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const 
 extern "C" int tnlm_cgls_step(tnlm_handle *H, const float *f_in, const float *y, const float *w, int m1,
                               float *g_out, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_cgls_step", n_slices, true);
+    int rc;
     if (!f_in || !y || !g_out) return fail(H, TNLM_INVALID_ARG, "f_in, y and g_out must not be NULL");
     if (m1 < 0) return fail(H, TNLM_INVALID_ARG, "m1 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
-    return cgls_device(H, f_in, y, w, m1, g_out, n_slices, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (m1 > 0 && (rc = prepare_sqrt_weights(H, w, n_slices, st))) return rc;
+    return cgls_device(H, f_in, y, w ? H->d_sw : nullptr, m1, g_out, n_slices, st);
 }
 
 // ------------------------------------------------------------------------------ TNLM
@@ -528,15 +652,12 @@ static const SweepShape *pick_shape(tnlm_handle *H, int n_img)
 {
     const SweepShape *best = nullptr;
     double best_cost = 0.0;
-    // tuning override for experiments: TNLM_SWEEP_SHAPE="rb,nb" restricts the choice
-    int want_rb = 0, want_nb = 0;
-    if (const char *ev = std::getenv("TNLM_SWEEP_SHAPE")) std::sscanf(ev, "%d,%d", &want_rb, &want_nb);
     for (const SweepShape &sh : H->shapes) {
-        if ((want_rb && sh.rb != want_rb) || (want_nb && sh.nb != want_nb)) continue;
+        if ((H->opt_rb && sh.rb != H->opt_rb) || (H->opt_nb && sh.nb != H->opt_nb)) continue;   // tuning override
         const double c = sweep_cost(H, sh, n_img);
         if (!best || c < best_cost) { best = &sh; best_cost = c; }
     }
-    if (!best) fail(H, TNLM_INVALID_ARG, "TNLM_SWEEP_SHAPE names a shape that is not available");
+    if (!best) fail(H, TNLM_INVALID_ARG, "option sweep_rb/sweep_nb (TNLM_SWEEP_SHAPE) names a shape that is not available");
     return best;
 }
 
@@ -561,6 +682,7 @@ static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, co
     const long long ctas = (long long)nimg * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
     void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out, (void *)&wts};
+    ProfScope ps(H, wts ? TNLM_KERNEL_SWEEP_STORE : TNLM_KERNEL_SWEEP, st);
     cudaError_t e = cudaLaunchKernel(wts ? sh.fn_store : sh.fn, dim3((unsigned)ctas), dim3(64 * sh.nb), args, sh.smem, st);
     if (e != cudaSuccess) return cuda_fail(H, e, "cudaLaunchKernel(gj_sweep_kernel)");
     LAUNCHED(H);
@@ -581,10 +703,8 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     const int threads = 32 * (sh.rb + 1);
     double best_eff = -1.0;
     size_t smem = 0;
-    int want_ns = 0;                                     // tuning override for experiments
-    if (const char *ev = std::getenv("TNLM_APPLY_NS")) want_ns = std::atoi(ev);
     for (int ns = AP_NS_MAX; ns >= 2; --ns) {
-        if (want_ns && ns != want_ns) continue;
+        if (H->opt_ns && ns != H->opt_ns) continue;      // tuning override
         const size_t sm = apply_smem_bytes(H->window, sh.rb, ns);
         if (sm > H->apply_smem) continue;
         const long long occ = std::min<long long>((long long)(H->smem_per_sm / (sm + 1024)), 2048 / threads);
@@ -594,6 +714,7 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
         if (eff > best_eff) { best_eff = eff; R.ap_ns = ns; smem = sm; }
     }
     if (best_eff < 0.0) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+    ProfScope ps(H, TNLM_KERNEL_APPLY, st);
     gj_apply_kernel<<<(unsigned)ctas, threads, smem, st>>>(R, g, u, out, wts);
     LAUNCHED(H);
     return TNLM_OK;
@@ -601,15 +722,13 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
 
 // Weight storage for m2 > 1: 2 bytes x 2 sides x W^2 per pixel of the padded band/tile grid.
 // Returns NULL (recompute every sweep instead) when that exceeds the cap
-// (TNLM_WEIGHT_CACHE_MB, default 16384; 0 disables).
+// (option weight_cache_mb / TNLM_WEIGHT_CACHE_MB, default 16384; 0 disables).
 static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices)
 {
-    size_t cap_mb = 16384;
-    if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) cap_mb = (size_t)std::strtoull(ev, nullptr, 10);
     SweepParams R = H->R;
     fill_layout(H, sh, R);
     const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
-    if (need * sizeof(__nv_bfloat16) > cap_mb * 1048576ull) return nullptr;
+    if (H->opt_cache_mb <= 0 || need * sizeof(__nv_bfloat16) > (size_t)H->opt_cache_mb * 1048576ull) return nullptr;
     if (need > H->wts_cap) {
         if (H->d_wts) cudaFree(H->d_wts);
         H->d_wts = nullptr; H->wts_cap = 0;
@@ -617,24 +736,6 @@ static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_s
         H->wts_cap = need;
     }
     return H->d_wts;
-}
-
-// Event pair around one kernel launch, on the launching stream.
-static int prof_mark(tnlm_handle *H, int kind, bool begin, cudaStream_t st)
-{
-    if (begin) {
-        const size_t need = 2 * H->prof_kind.size() + 2;
-        while (H->prof_ev.size() < need) {
-            cudaEvent_t e;
-            CU(H, cudaEventCreate(&e));
-            H->prof_ev.push_back(e);
-        }
-        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size()], st));
-        H->prof_kind.push_back(kind);
-    } else {
-        CU(H, cudaEventRecord(H->prof_ev[2 * H->prof_kind.size() - 1], st));
-    }
-    return TNLM_OK;
 }
 
 extern "C" int tnlm_fma_peak(double *tflops, void *stream)
@@ -669,7 +770,7 @@ extern "C" int tnlm_fma_peak(double *tflops, void *stream)
     return TNLM_OK;
 }
 
-extern "C" int tnlm_profile_sweeps(tnlm_handle *H, int enable)
+extern "C" int tnlm_profile_kernels(tnlm_handle *H, int enable)
 {
     if (!H) return TNLM_INVALID_ARG;
     H->err.clear();
@@ -678,11 +779,12 @@ extern "C" int tnlm_profile_sweeps(tnlm_handle *H, int enable)
     return TNLM_OK;
 }
 
-extern "C" int tnlm_sweep_times(tnlm_handle *H, float *ms, int *kind, int capacity, int *count)
+extern "C" int tnlm_kernel_times(tnlm_handle *H, float *ms, int *kind, int capacity, int *count)
 {
     if (!H) return TNLM_INVALID_ARG;
     H->err.clear();
     if (!count || capacity < 0 || (capacity > 0 && (!ms || !kind))) return fail(H, TNLM_INVALID_ARG, "count, and ms/kind when capacity > 0, must not be NULL");
+    DeviceGuard dg(H->device);
     const int n = (int)H->prof_kind.size();
     *count = n;
     for (int i = 0; i < n && i < capacity; ++i) {
@@ -694,19 +796,43 @@ extern "C" int tnlm_sweep_times(tnlm_handle *H, float *ms, int *kind, int capaci
     return TNLM_OK;
 }
 
+extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value)
+{
+    if (!H) return TNLM_INVALID_ARG;
+    H->err.clear();
+    if (!name) return fail(H, TNLM_INVALID_ARG, "option name is NULL");
+    const std::string n(name);
+    if (n == "weight_cache_mb") H->opt_cache_mb = value;
+    else if (n == "sweep_rb") H->opt_rb = (int)value;
+    else if (n == "sweep_nb") H->opt_nb = (int)value;
+    else if (n == "apply_ns") H->opt_ns = (int)value;
+    else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);
+    return TNLM_OK;
+}
+
+extern "C" int tnlm_device(const tnlm_handle *H) { return H ? H->device : -1; }
+
+static int regularize_workspace(tnlm_handle *H, int m2, bool alias)
+{
+    int rc;
+    if (m2 > 1 || alias) if ((rc = need(H, &H->d_ua, img_count(H)))) return rc;
+    if (m2 > 2 || (alias && m2 > 1)) if ((rc = need(H, &H->d_ub, img_count(H)))) return rc;
+    return TNLM_OK;
+}
+
 // g -> f_out; g and f_out are distinct device buffers or the same buffer.
 static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_out, int n_slices, cudaStream_t st)
 {
     const size_t n = (size_t)n_slices * H->n_phase * H->nx * H->ny;
     int rc;
     if (m2 == 0) {
+        ProfScope ps(H, TNLM_KERNEL_CLIP, st);
         clip_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, f_out, n);
         LAUNCHED(H);
         return TNLM_OK;
     }
     const bool alias = (f_out == g);
-    if (m2 > 1 || alias) if ((rc = need(H, &H->d_ua, img_count(H)))) return rc;
-    if (m2 > 2 || (alias && m2 > 1)) if ((rc = need(H, &H->d_ub, img_count(H)))) return rc;
+    if ((rc = regularize_workspace(H, m2, alias))) return rc;
     const float *src = g;
     float *pp[2] = {H->d_ua, H->d_ub};
     int which = 0;
@@ -719,12 +845,9 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
         if (last && !alias) dst = f_out;
         else { dst = pp[which]; if (dst == src) { which ^= 1; dst = pp[which]; } }
         const bool computes = (m == 0 || !wts);
-        const int kind = computes ? (wts ? TNLM_KERNEL_SWEEP_STORE : TNLM_KERNEL_SWEEP) : TNLM_KERNEL_APPLY;
-        if (H->prof && (rc = prof_mark(H, kind, true, st))) return rc;
         if (computes) rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
         else rc = launch_apply(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
         if (rc) return rc;
-        if (H->prof && (rc = prof_mark(H, kind, false, st))) return rc;
         src = dst;
         which ^= 1;
     }
@@ -734,8 +857,8 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
 
 extern "C" int tnlm_regularize_step(tnlm_handle *H, const float *g, int m2, float *f_out, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, false);
-    if (rc) return rc;
+    ENTER(H, "tnlm_regularize_step", n_slices, false);
+    int rc;
     if (!g || !f_out) return fail(H, TNLM_INVALID_ARG, "g and f_out must not be NULL");
     if (m2 < 0) return fail(H, TNLM_INVALID_ARG, "m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
@@ -752,8 +875,10 @@ static int reconstruct_device(tnlm_handle *H, const float *y, const float *w, co
     else CU(H, cudaMemsetAsync(f_out, 0, n * sizeof(float), st));
     if (k_outer == 0) return TNLM_OK;
     if ((rc = need(H, &H->d_g, img_count(H)))) return rc;
+    if (m1 > 0 && (rc = prepare_sqrt_weights(H, w, n_slices, st))) return rc;
+    const float *sw = w ? H->d_sw : nullptr;
     for (int k = 0; k < k_outer; ++k) {
-        if ((rc = cgls_device(H, f_out, y, w, m1, H->d_g, n_slices, st))) return rc;       // step 2 (L176)
+        if ((rc = cgls_device(H, f_out, y, sw, m1, H->d_g, n_slices, st))) return rc;      // step 2 (L176)
         if ((rc = regularize_device(H, H->d_g, m2, f_out, n_slices, st))) return rc;       // steps 3-5
     }
     return TNLM_OK;
@@ -762,19 +887,45 @@ static int reconstruct_device(tnlm_handle *H, const float *y, const float *w, co
 extern "C" int tnlm_reconstruct(tnlm_handle *H, const float *y, const float *w, const float *f0, int k_outer, int m1,
                                 int m2, float *f_out, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_reconstruct", n_slices, true);
+    int rc;
     if (!y || !f_out) return fail(H, TNLM_INVALID_ARG, "y and f_out must not be NULL");
     if (k_outer < 0 || m1 < 0 || m2 < 0) return fail(H, TNLM_INVALID_ARG, "k_outer, m1, m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
     return reconstruct_device(H, y, w, f0, k_outer, m1, m2, f_out, n_slices, (cudaStream_t)stream);
 }
 
+// All allocation a later call with these parameters would do, done now (cudaMalloc synchronises the device;
+// after tnlm_reserve the enqueue calls with n_slices, m1, m2 up to the reserved ones never allocate).
+extern "C" int tnlm_reserve(tnlm_handle *H, int n_slices, int m1, int m2, int host_entry_points)
+{
+    ENTER(H, "tnlm_reserve", n_slices, false);
+    int rc;
+    if (m1 < 0 || m2 < 0) return fail(H, TNLM_INVALID_ARG, "m1, m2 must be >= 0");
+    if ((rc = ensure_ws(H, n_slices))) return rc;
+    if ((rc = regularize_workspace(H, m2, true))) return rc;
+    if (m2 > 1) {
+        const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
+        if (!sh) return TNLM_INVALID_ARG;
+        weight_cache(H, *sh, n_slices);              // NULL (over the cap) just means "recompute"
+    }
+    if ((rc = need(H, &H->d_g, img_count(H)))) return rc;
+    if (host_entry_points && (rc = need(H, &H->d_f, img_count(H)))) return rc;
+    if (H->has_geom) {
+        if ((rc = cgls_workspace(H, std::max(m1, 1), n_slices, true))) return rc;
+        if (host_entry_points) {
+            if ((rc = need(H, &H->d_yh, sino_count(H)))) return rc;
+            if ((rc = need(H, &H->d_wh, sino_count(H)))) return rc;
+        }
+    }
+    return TNLM_OK;
+}
+
 // ------------------------------------------------------------------------------ host-buffer entry points
 extern "C" int tnlm_regularize_step_host(tnlm_handle *H, const float *g_host, int m2, float *f_out_host, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, false);
-    if (rc) return rc;
+    ENTER(H, "tnlm_regularize_step_host", n_slices, false);
+    int rc;
     if (!g_host || !f_out_host) return fail(H, TNLM_INVALID_ARG, "g_host and f_out_host must not be NULL");
     if (m2 < 0) return fail(H, TNLM_INVALID_ARG, "m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
@@ -792,8 +943,8 @@ extern "C" int tnlm_regularize_step_host(tnlm_handle *H, const float *g_host, in
 extern "C" int tnlm_reconstruct_host(tnlm_handle *H, const float *y_host, const float *w_host, const float *f0_host,
                                      int k_outer, int m1, int m2, float *f_out_host, int n_slices, void *stream)
 {
-    int rc = check_common(H, n_slices, true);
-    if (rc) return rc;
+    ENTER(H, "tnlm_reconstruct_host", n_slices, true);
+    int rc;
     if (!y_host || !f_out_host) return fail(H, TNLM_INVALID_ARG, "y_host and f_out_host must not be NULL");
     if (k_outer < 0 || m1 < 0 || m2 < 0) return fail(H, TNLM_INVALID_ARG, "k_outer, m1, m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
