@@ -49,7 +49,8 @@ class Geometry:
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libtnlm.so")
+    """The in-tree library; TNLM_LIBRARY names another build of it (kernel experiments)."""
+    return os.environ.get("TNLM_LIBRARY") or os.path.join(_HERE, "libtnlm.so")
 
 
 def library():

@@ -7,7 +7,7 @@ namespace tnlm {
 
 // Ray table entry, one per (phase, view, bin); built once in tnlm_create from the geometry in
 // double precision.  Both projector kernels read the SAME entry and run the SAME fp32
-// expressions on it (ray_cell below), so P^T is the exact transpose of P entry by entry.
+// expressions on it (ray_cum below), so P^T is the exact transpose of P entry by entry.
 //   steep ray (|dy| >= |dx|): column coordinate xi(eta) = p0 + m*eta   (grid units, pixel c = [c,c+1))
 //   shallow ray             : row    coordinate eta(xi) = p0 + m*xi
 //   plo  = p0 + min(m, 0): the smaller of the two coordinates at which the ray enters / leaves
@@ -36,28 +36,30 @@ struct Geom {
 constexpr float FLOOR_MAGIC = 12582912.0f;
 constexpr int FLOOR_MAGIC_BITS = 0x4B400000;
 
-// One row (steep) or column (shallow) of one ray: the at most two cells it touches there and the
-// lengths inside them.  qf = row index (steep) / column index (shallow) as a float.  Returns c0 (the
-// cell holding the smaller coordinate; the other cell, if any, is c0+1) and w0, w1 (mm); w1 == 0
-// when the ray stays in one cell.  The split is at the cell boundary b = c0+1: the fraction of the
-// crossing below b is sat((b - lo)/|m|), which is 1 when the ray does not reach b.  Explicit
-// intrinsics: no contraction differences between the two kernels that inline this.
-__device__ __forceinline__ void ray_cell_f(const float plo, const float m, const float alen, const float inva,
-                                           const float qf, float &f0r, float &f0, float &w0, float &w1)
+// One row (steep) or column (shallow) q of one ray crosses the minor axis over [lo, lo + |m|], |m| <= 1,
+// lo = m*q + plo, so it touches at most the two cells c0 = floor(lo) and c0 + 1.  With the cumulative
+// fraction of the crossing that lies below coordinate b,
+//     F(b) = sat( ((b - 1) - lo) * inva + inva ),          inva = 1/|m|   (1e30 for m = 0: a step function)
+// the CANONICAL matrix entry both projectors produce is
+//     P[ray, (q, c)] = fl( alen * fl( F(c+1) - F(c) ) ),    alen = length of the ray inside one full row (mm).
+// F is exactly 0 for b <= c0 and exactly 1 for b >= c0 + 2, so only F(c0 + 1) is fractional: the forward
+// projector evaluates just that one (ray_frac: F1 and U1 = 1 - F1 are the fractions of cells c0 and c0 + 1),
+// the gather evaluates F at the three boundaries of its two pixels with the SAME expression (ray_cum), and
+// every entry is bit-identical on the two sides: P^T is the exact transpose of P.
+// Explicit intrinsics: no contraction differences between the two kernels that inline these.
+__device__ __forceinline__ float ray_lo(const float plo, const float m, const float qf) { return __fmaf_rn(m, qf, plo); }
+__device__ __forceinline__ float ray_cum(const float bm1, const float lo, const float inva)
 {
-    const float lo = __fmaf_rn(m, qf, plo);
-    f0r = __fadd_rd(lo, FLOOR_MAGIC);                                  // bits: FLOOR_MAGIC_BITS + floor(lo)
-    f0 = __fsub_rn(f0r, FLOOR_MAGIC);                                  // floor(lo) as a float, exactly
-    const float t = __fsub_rn(f0, lo);                                 // floor(lo) - lo in (-1, 0]
-    const float frac = __saturatef(__fmaf_rn(t, inva, inva));          // ((c0+1) - lo)/|m|, clamped
-    w0 = __fmul_rn(alen, frac);
-    w1 = __fsub_rn(alen, w0);
+    return __saturatef(__fmaf_rn(__fsub_rn(bm1, lo), inva, inva));
 }
-__device__ __forceinline__ void ray_cell(const float plo, const float m, const float alen, const float inva,
-                                         const float qf, int &c0, float &w0, float &w1)
+__device__ __forceinline__ void ray_frac(const float plo, const float m, const float inva, const float qf, int &c0,
+                                         float &F1, float &U1)
 {
-    float f0r, f0;
-    ray_cell_f(plo, m, alen, inva, qf, f0r, f0, w0, w1);
+    const float lo = ray_lo(plo, m, qf);
+    const float f0r = __fadd_rd(lo, FLOOR_MAGIC);                      // bits: FLOOR_MAGIC_BITS + floor(lo)
+    const float f0 = __fsub_rn(f0r, FLOOR_MAGIC);                      // floor(lo) as a float, exactly
+    F1 = ray_cum(f0, lo, inva);                                        // F(c0 + 1)
+    U1 = __fsub_rn(1.0f, F1);                                          // F(c0 + 2) - F(c0 + 1)
     c0 = __float_as_int(f0r) - FLOOR_MAGIC_BITS;
 }
 

@@ -1,7 +1,7 @@
 // projector.cuh -- fan-beam forward projector P (ray-driven, one thread per (view,bin)) and its
 // matched adjoint P^T (pixel-driven gather, one thread per pixel).  PAPER.md:L75, L79, L212.
-// Both kernels evaluate tnlm::ray_cell on the same RayEntry table, so every matrix entry
-// len(ray ∩ pixel) is bit-identical on the two sides and P^T is the exact transpose of P.
+// Both kernels evaluate tnlm::ray_cum on the same RayEntry table, so every matrix entry
+// len(ray ∩ pixel) is bit-identical on the two sides and P^T is the exact transpose of P (common.cuh).
 #pragma once
 #include "common.cuh"
 
@@ -17,7 +17,7 @@ enum FwdMode {
 // atan on the fan-angle range: odd minimax polynomial on [-1, 1] (Abramowitz & Stegun 4.4.49,
 // |error| <= 2e-8 rad, i.e. < 1e-4 bin); detectors wider than +-40 degrees use atanf (kernel
 // template POLY = false).  Only the conservative candidate range of the backprojector depends on
-// it; membership and lengths come from ray_cell.
+// it; membership and lengths come from ray_cum.
 __device__ __forceinline__ float fan_angle_poly(float t)
 {
     const float z = t * t;
@@ -74,7 +74,7 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
         const RayEntry e = tab[(size_t)phase * nray + ray];
         const RayRange rg = rng[(size_t)phase * nray + ray];
         const float alen = fabsf(e.len);
-        float acc0 = 0.f, acc1 = 0.f;
+        float acc0 = 0.f, acc1 = 0.f;                            // sums of fraction x pixel value; x alen once at the end
         // steep rays walk the rows of the image, shallow rays the rows of the transposed image
         const bool steep = e.len > 0.f;
         const int n_minor = steep ? G.nx : G.ny;             // length of a walked row
@@ -83,10 +83,10 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
             float qf = (float)q0;
             const float *__restrict__ row = base + (size_t)q0 * n_minor;
             for (int q = q0; q <= q1; ++q, qf += 1.0f, row += n_minor) {
-                int c0; float w0, w1;
-                ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
-                if ((unsigned)c0 < (unsigned)n_minor) acc0 = fmaf(w0, __ldg(row + c0), acc0);
-                if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
+                int c0; float F1, U1;
+                ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+                if ((unsigned)c0 < (unsigned)n_minor) acc0 = fmaf(F1, __ldg(row + c0), acc0);
+                if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1 = fmaf(U1, __ldg(row + c0 + 1), acc1);
             }
         };
         if (rg.ihi >= rg.ilo) {
@@ -95,16 +95,16 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
             const float *__restrict__ row = base + (size_t)rg.ilo * n_minor;
 #pragma unroll 4
             for (int q = rg.ilo; q <= rg.ihi; ++q, qf += 1.0f, row += n_minor) {
-                int c0; float w0, w1;
-                ray_cell(e.plo, e.m, alen, e.inva, qf, c0, w0, w1);
-                acc0 = fmaf(w0, __ldg(row + c0), acc0);
-                acc1 = fmaf(w1, __ldg(row + c0 + 1), acc1);
+                int c0; float F1, U1;
+                ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+                acc0 = fmaf(F1, __ldg(row + c0), acc0);
+                acc1 = fmaf(U1, __ldg(row + c0 + 1), acc1);
             }
             edge(rg.ihi + 1, rg.hi);
         } else {
             edge(rg.lo, rg.hi);
         }
-        const float p = acc0 + acc1;
+        const float p = __fmul_rn(alen, acc0 + acc1);
         const size_t o = (size_t)prob * nray + ray;
         if (MODE == FWD_PLAIN) {
             out0[o] = p;
@@ -139,7 +139,7 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
 // (rows r0, r0+1, columns c0, c0+1; a warp covers 16 x 8 pixels), loop over the views of its
 // phase.  Per view the candidate bins are those whose fan angle is within the block's angular
 // footprint (conservative superset).  A steep candidate is evaluated in rows r0 and r0+1, a
-// shallow one in columns c0 and c0+1: each ray_cell serves the two block pixels of that row
+// shallow one in columns c0 and c0+1: each evaluation serves the two block pixels of that row
 // (column), so the block costs 2 evaluations per candidate instead of 4, and the same expressions
 // as the forward projector decide membership and give the lengths (exact transpose).
 // red (optional) += ||out||^2 of this problem.
@@ -160,7 +160,7 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
         // block centre
         const float X = ((float)c0 + 0.5f - 0.5f * (float)(G.nx - 1)) * G.pix;
         const float Y = ((float)r0 + 0.5f - 0.5f * (float)(G.ny - 1)) * G.pix;
-        const float rf = (float)r0, cf = (float)c0, dcr = cf - rf;
+        const float rf = (float)r0, cf = (float)c0, dcr = cf - rf, rfm1 = rf - 1.0f;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
         const float4 *__restrict__ tb = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg = sino + (size_t)prob * V * B;
@@ -179,35 +179,32 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const float4 *__restrict__ tbk = tb + k_lo;
             const float *__restrict__ sgk = sg + k_lo;
-            // Membership and lengths by FP32-pipe arithmetic (the integer / compare pipe is half rate
-            // and was the bottleneck): st = 1 for a steep ray, 0 for a shallow one; evaluation j is in
-            // row r0+j (steep) or column c0+j (shallow); with dm = (index of the block's first pixel
-            // along the other axis) - floor(lo): that pixel holds w0 if dm = 0, w1 if dm = 1, and its
-            // neighbour holds w0 if dm = -1, w1 if dm = 0.
+            // Membership and lengths by FP32-pipe arithmetic only: st = 1 for a steep ray, 0 for a shallow one;
+            // evaluation j is in row r0+j (steep) or column c0+j (shallow); the block's two pixels in that line
+            // sit at minor-axis indices cA and cA+1 (cA = c0 steep, r0 shallow) and get
+            // alen * (F(cA+1) - F(cA)) and alen * (F(cA+2) - F(cA+1)), F = ray_cum (common.cuh): zero for cells
+            // the ray misses, and bit for bit the forward projector's entry for the cells it touches.
             for (int n = k_hi - k_lo; n >= 0; --n, ++tbk, ++sgk) {
                 const float4 e4 = __ldg(tbk);                // plo, m, len (sign = steep), inva
                 const float sv = __ldg(sgk);
                 const float st = __saturatef(e4.z * 1.0e30f);
                 const float qf = __fmaf_rn(st, -dcr, cf);    // rf (steep) or cf (shallow), exactly
-                const float mef = __fmaf_rn(st, dcr, rf);    // cf (steep) or rf (shallow), exactly
-                const float alen = fabsf(e4.z);
-                float wA[2], wB[2];
+                const float me0 = __fmaf_rn(st, dcr, rfm1);  // cA - 1: cf - 1 (steep) or rf - 1 (shallow), exactly
+                const float me1 = me0 + 1.0f, me2 = me0 + 2.0f;
+                const float asv = __fmul_rn(fabsf(e4.z), sv);
+                float dA[2], dB[2];
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    float f0r, f0, w0, w1;
-                    ray_cell_f(e4.x, e4.y, alen, e4.w, qf + (float)j, f0r, f0, w0, w1);
-                    const float dm = __fsub_rn(mef, f0);
-                    const float i0 = __saturatef(1.0f - fabsf(dm));
-                    const float i1 = __saturatef(1.0f - fabsf(dm - 1.0f));
-                    const float im = __saturatef(1.0f - fabsf(dm + 1.0f));
-                    wA[j] = __fmaf_rn(w0, i0, __fmul_rn(w1, i1));     // w0, w1 or 0, exactly
-                    wB[j] = __fmaf_rn(w0, im, __fmul_rn(w1, i0));
+                    const float lo = ray_lo(e4.x, e4.y, qf + (float)j);
+                    const float G0 = ray_cum(me0, lo, e4.w), G1 = ray_cum(me1, lo, e4.w), G2 = ray_cum(me2, lo, e4.w);
+                    dA[j] = __fsub_rn(G1, G0);
+                    dB[j] = __fsub_rn(G2, G1);
                 }
                 const bool steep = e4.z > 0.f;
-                a00 = fmaf(wA[0], sv, a00);
-                a11 = fmaf(wB[1], sv, a11);
-                a01 = fmaf(steep ? wB[0] : wA[1], sv, a01);
-                a10 = fmaf(steep ? wA[1] : wB[0], sv, a10);
+                a00 = __fmaf_rn(asv, dA[0], a00);
+                a11 = __fmaf_rn(asv, dB[1], a11);
+                a01 = __fmaf_rn(asv, steep ? dB[0] : dA[1], a01);
+                a10 = __fmaf_rn(asv, steep ? dA[1] : dB[0], a10);
             }
         }
         float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + (size_t)r0 * G.nx + c0;

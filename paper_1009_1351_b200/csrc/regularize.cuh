@@ -34,9 +34,11 @@
 // Stored weights ("reusing this factor ... instead of recomputing").  The weights
 // belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 the first sweep
 // (STORE_W = true) also writes every unnormalised weight as bf16 into
-// wts[image][side][band][tile_x][delta][RB rows][128 columns] -- one contiguous chunk per warp
-// band, written and later read as a sequential stream (DRAM-page friendly; a plane-per-offset
-// layout scatters 256-byte pieces and ran 3x slower).  bf16 keeps the fp32 exponent range, so the
+// wts[image][side][band][tile_x][delta][RB/2 row pairs][32 lanes][2 rows][4 columns] -- one
+// contiguous chunk per warp band, written and later read as a sequential stream (DRAM-page
+// friendly; a plane-per-offset layout scatters 256-byte pieces and ran 3x slower); inside a plane
+// the two rows of a pair are interleaved per lane so that the applying sweeps read 16 bytes per
+// lane (plane_off below).  bf16 keeps the fp32 exponent range, so the
 // stored values are the very 2^(c(D0-D)-100) of the fast path (an fp16 version needed its own
 // reference and sent every moving edge through the slow exact route: 2.6x slower); the quotient
 // A/Z of Eq. (7) does not depend on the per-pixel scale, and the 2^-9 rounding of each weight
@@ -79,6 +81,7 @@ struct SweepParams {
     float a_limit;          // ... or whose numerator magnitude is not below this (2^120)
     int clip;               // apply max(.,0) to the output
     int ap_ns;              // gj_apply_kernel: stages of its bulk-copy ring
+    int n_img;              // gj_apply2_kernel: S*N images in this launch
 };
 
 // Shared-memory tile geometry (words), shared by host (sizing) and device.
@@ -98,6 +101,12 @@ struct SweepGeom {
     }
 };
 
+// Position (in halves) of pixel (band row rr, tile column cc) inside one stored-weight plane of RB x 128.
+__host__ __device__ __forceinline__ int plane_off(int rr, int cc)
+{
+    return ((((rr >> 1) << 5) + (cc >> 2)) << 3) + ((rr & 1) << 2) + (cc & 3);
+}
+
 __device__ __forceinline__ float fast_ex2(float t)
 {
     float e;
@@ -105,11 +114,30 @@ __device__ __forceinline__ float fast_ex2(float t)
     return e;
 }
 
-// Zero-filled copy of the image window rows [r_org, r_org+rows) x cols [c_org, c_org+width)
-// into dst[rows][width]; warps take rows, lanes take columns (coalesced).
-__device__ __forceinline__ void load_tile(float *__restrict__ dst, int rows, int width,
-                                          const float *__restrict__ img, int r_org, int c_org, int ny, int nx,
-                                          int warp, int nwarps, int lane)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// ---- cp.async (LDGSTS): global -> shared copies that hold no registers while in flight -----------------
+// 4-byte copy; `valid` false writes 0.0f instead (src-size 0: nothing is read).
+__device__ __forceinline__ void cp_async4_zfill(void *dst, const void *src, bool valid)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 4 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Zero-filled copy of the image window rows [r_org, r_org+rows) x cols [c_org, c_org+width) into
+// dst[rows][width]; warps take rows, lanes take columns (coalesced).  Asynchronous: every element is its
+// own cp.async, so all of a tile's loads are in flight together (a load-then-store loop exposed one L2
+// round trip per row and lane: 13 us per CTA of the sweep, 7-14 us per CTA of the stored-weight sweep).
+// The caller commits the group, waits for it and synchronises the threads that read the tile.
+__device__ __forceinline__ void stage_tile_async(float *__restrict__ dst, int rows, int width,
+                                                 const float *__restrict__ img, int r_org, int c_org, int ny, int nx,
+                                                 int warp, int nwarps, int lane)
 {
     for (int rr = warp; rr < rows; rr += nwarps) {
         const int r = r_org + rr;
@@ -118,7 +146,8 @@ __device__ __forceinline__ void load_tile(float *__restrict__ dst, int rows, int
         float *__restrict__ d = dst + rr * width;
         for (int cc = lane; cc < width; cc += 32) {
             const int c = c_org + cc;
-            d[cc] = (rin && (unsigned)c < (unsigned)nx) ? __ldg(src + c) : 0.f;
+            const bool in = rin && (unsigned)c < (unsigned)nx;
+            cp_async4_zfill(d + cc, src + (in ? c : 0), in);
         }
     }
 }
@@ -208,16 +237,18 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 
     {   // stage g_i, and g_j / u_j of both cyclic neighbours (L81), zero-filled outside the image
         const float *__restrict__ gi = g + (size_t)img * npix;
-        load_tile(sGi, gi_rows, GIW, gi, tile_r0 - PB, tile_c0 - PB, ny, nx, warp, nwarps, lane);
+        stage_tile_async(sGi, gi_rows, GIW, gi, tile_r0 - PB, tile_c0 - PB, ny, nx, warp, nwarps, lane);
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
             const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
             const size_t jo = ((size_t)slice * p.n_phase + j) * npix;
-            load_tile(sGj + s * gj_rows * GJW, gj_rows, GJW, g + jo, tile_r0 - PB - a, tile_c0 - PB - a, ny, nx,
-                      warp, nwarps, lane);
-            load_tile(sUj + s * uj_rows * UJW, uj_rows, UJW, u + jo, tile_r0 - a, tile_c0 - a, ny, nx, warp,
-                      nwarps, lane);
+            stage_tile_async(sGj + s * gj_rows * GJW, gj_rows, GJW, g + jo, tile_r0 - PB - a, tile_c0 - PB - a, ny, nx,
+                             warp, nwarps, lane);
+            stage_tile_async(sUj + s * uj_rows * UJW, uj_rows, UJW, u + jo, tile_r0 - a, tile_c0 - a, ny, nx, warp,
+                             nwarps, lane);
         }
+        cp_async_commit();
+        cp_async_wait<0>();
     }
     __syncthreads();
 
@@ -305,7 +336,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             const float4 *__restrict__ ujp = reinterpret_cast<const float4 *>(myUj + (lr0 + dr + a) * UJW) + lane + dcg;
             const float4 *__restrict__ kp = reinterpret_cast<const float4 *>(myK) + lane;
             __nv_bfloat16 *__restrict__ witem =
-                STORE_W ? wchunk + ((size_t)(dr + a) * (2 * a + 1) + (dc0 + a)) * WSTRIDE + C * lane : nullptr;
+                STORE_W ? wchunk + ((size_t)(dr + a) * (2 * a + 1) + (dc0 + a)) * WSTRIDE + 8 * lane : nullptr;
 #pragma unroll
             for (int s = 0; s < RB + 2 * PB; ++s) {
                 float gi_[4 * NGI], gj_[4 * NGJ];
@@ -373,7 +404,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         pk.x = *reinterpret_cast<const unsigned *>(&lo);
                         pk.y = *reinterpret_cast<const unsigned *>(&hi);
                         if (dc0 + gg <= a)         // (rows / columns past the image edge land in chunk padding)
-                            *reinterpret_cast<uint2 *>(witem + gg * WSTRIDE + rr * SW_TW) = pk;
+                            *reinterpret_cast<uint2 *>(witem + gg * WSTRIDE + (rr >> 1) * 256 + (rr & 1) * 4) = pk;
                     }
                 }
                 SW_STEP_FENCE();
@@ -395,7 +426,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             while (m) {
                 const int L = __ffs(m) - 1;
                 m &= m - 1;
-                __nv_bfloat16 *wpix = STORE_W ? wchunk + rr * SW_TW + C * L + c : nullptr;
+                __nv_bfloat16 *wpix = STORE_W ? wchunk + plane_off(rr, C * L + c) : nullptr;
                 __syncwarp();                      // the fast path's stores to this pixel come first
                 const float v = exact_side_ratio<PB>(sGi, myGj, myUj, GJW, UJW, lr0 + rr, C * L + c, r0 + rr,
                                                      tile_c0 + C * L + c, a, ny, nx, p.neg_c, lane, wpix, WSTRIDE);
@@ -439,7 +470,6 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 }
 
 // ---- mbarrier / bulk-copy (TMA) primitives used by gj_apply_kernel -----------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
@@ -554,9 +584,11 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
         const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
-        load_tile(sU + s * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a,
-                  tile_c0 - a, ny, nx, warp, rb, lane);
+        stage_tile_async(sU + s * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a,
+                         tile_c0 - a, ny, nx, warp, rb, lane);
     }
+    cp_async_commit();
+    cp_async_wait<0>();
     asm volatile("bar.sync 1, %0;" ::"r"(32 * rb) : "memory");      // consumers only
 
     const int r = tile_r0 + warp, c0 = tile_c0 + C * lane;
@@ -575,7 +607,7 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                 const float uw[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
                 const int noff = min(AP_SO, W - AP_SO * k);
                 mbar_wait(full + slot, parity);
-                const uint2 *__restrict__ wq = reinterpret_cast<const uint2 *>(sW + (size_t)slot * AP_SO * wstride + warp * SW_TW) + lane;
+                const uint2 *__restrict__ wq = reinterpret_cast<const uint2 *>(sW + (size_t)slot * AP_SO * wstride + plane_off(warp, C * lane));
                 uint2 wv[AP_SO];
 #pragma unroll
                 for (int jj = 0; jj < AP_SO; ++jj) wv[jj] = wq[(jj < noff ? jj : 0) * (wstride / 4)];
@@ -610,6 +642,134 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             if (p.clip) v = fmaxf(v, 0.f);
             o[c] = v;
         }
+}
+
+// The same sweep as a persistent, warp-task kernel (the default).  A task = one ROW PAIR of one stored band
+// (2 rows x 128 columns, both sides): the 2*W^2 pieces of 512 bytes that hold its weights (the row-pair
+// interleave of the stored layout makes a warp's piece contiguous, 16 bytes per lane).  Tasks are dealt
+// round-robin to all resident warps of the device, so every SM streams the same number of bytes to within one
+// task.  A warp is self-contained: it stages its own u_j window (2+2a rows) and keeps DEPTH pieces in flight in a
+// private ring, all with cp.async (LDGSTS: no registers held by loads in flight, no mbarriers, no producer
+// warp), and never synchronises with another warp.  Measured on the box: a 322 MB
+// read-only stream of this shape runs at 6.2 TB/s; what kept the first versions at 4.4 TB/s was the u_j tile
+// staging (a load-then-store loop: one exposed L2 round trip per row), not the stream.
+// grid.x = resident CTAs (host: n_sm x CTAs per SM); block = 32 x warps per CTA (host's choice);
+// dynamic smem = warps x apply2_warp_bytes.
+__host__ __device__ inline size_t apply2_warp_bytes(int window, int depth)
+{
+    const int a = (window - 1) / 2;
+    return (size_t)(2 + 2 * a) * apply_uw(window) * sizeof(float) + (size_t)depth * 512;
+}
+
+template <int DEPTH>             // pieces in flight per warp (a power of two)
+__global__ void __launch_bounds__(256, 2)
+gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
+                 const __nv_bfloat16 *__restrict__ wts)
+{
+    constexpr int C = SW_C;
+    const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1, WW = W * W;
+    const int UW = apply_uw(W), urows = 2 + 2 * a;
+    const int rb = p.rb, npairs = rb >> 1;
+    const size_t pstride = (size_t)rb * (SW_TW / 8);     // uint4 per offset plane
+    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)WW * pstride;      // uint4
+    const size_t npix = (size_t)nx * ny;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
+    extern __shared__ float4 smem4[];
+    const size_t wbytes = apply2_warp_bytes(W, DEPTH);
+    float *sU = reinterpret_cast<float *>(reinterpret_cast<char *>(smem4) + warp * wbytes);   // [urows][UW]
+    uint4 *ring = reinterpret_cast<uint4 *>(sU + urows * UW) + lane;                          // [DEPTH][32 lanes]
+
+    const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
+    const long long n_tasks = (long long)p.n_img * tiles_per_img * npairs;
+    const long long n_warps = (long long)gridDim.x * wpc;
+#pragma unroll 1
+    for (long long task = (long long)blockIdx.x * wpc + warp; task < n_tasks; task += n_warps) {
+        const int pair = (int)(task % npairs);
+        const long long chunk = task / npairs;               // (img, gband, tx)
+        const int img = (int)(chunk / tiles_per_img);
+        const int tl = (int)(chunk - (long long)img * tiles_per_img);
+        const int gband = tl / p.tiles_x, tx = tl - gband * p.tiles_x;
+        const int r = gband * rb + 2 * pair, tile_c0 = tx * SW_TW, c0 = tile_c0 + C * lane;
+        const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
+        const uint4 *__restrict__ wp = reinterpret_cast<const uint4 *>(wts) +
+                                       ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)WW * pstride +
+                                       pair * 32 + lane;
+        float nbsum[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll 1
+        for (int sd = 0; sd < 2; ++sd) {
+            const uint4 *__restrict__ ws = wp + sd * side_stride;
+            const int j = (phase + (sd == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
+            __syncwarp();                                     // the previous window is no longer read
+            // oldest group: this side's u_j window; then pieces 0..DEPTH-2 of its weights
+            stage_tile_async(sU, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, r - a, tile_c0 - a, ny, nx, 0, 1, lane);
+            cp_async_commit();
+#pragma unroll 1
+            for (int t = 0; t < DEPTH - 1; ++t) {
+                if (t < WW) cp_async16(ring + (t % DEPTH) * 32, ws + (size_t)t * pstride);
+                cp_async_commit();
+            }
+            cp_async_wait<DEPTH - 1>();                       // the window has landed (every lane's part of it)
+            __syncwarp();
+            float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+            int t = 0;
+#pragma unroll 1
+            for (int dr = 0; dr < W; ++dr) {
+                const float *__restrict__ urow0 = sU + dr * UW + C * lane;
+#pragma unroll 1
+                for (int k = 0; k < W; k += 4) {
+                    const float4 ua = *reinterpret_cast<const float4 *>(urow0 + k), ub = *reinterpret_cast<const float4 *>(urow0 + k + 4);
+                    const float4 uc = *reinterpret_cast<const float4 *>(urow0 + UW + k), ud = *reinterpret_cast<const float4 *>(urow0 + UW + k + 4);
+                    const float uw0[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
+                    const float uw1[8] = {uc.x, uc.y, uc.z, uc.w, ud.x, ud.y, ud.z, ud.w};
+                    const int noff = min(4, W - k);
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        if (jj < noff) {
+                            const int tn = t + DEPTH - 1;
+                            if (tn < WW) cp_async16(ring + (tn % DEPTH) * 32, ws + (size_t)tn * pstride);
+                            cp_async_commit();                // (empty groups keep the wait count uniform)
+                            cp_async_wait<DEPTH - 1>();       // piece t has landed (this lane's own 16 bytes)
+                            const uint4 wv = ring[(t % DEPTH) * 32];
+                            ++t;
+                            // bf16 -> fp32 is a 16-bit shift: low half << 16, high half masked
+                            const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
+                                                 __uint_as_float(wv.y << 16), __uint_as_float(wv.y & 0xffff0000u)};
+                            const float w1[C] = {__uint_as_float(wv.z << 16), __uint_as_float(wv.z & 0xffff0000u),
+                                                 __uint_as_float(wv.w << 16), __uint_as_float(wv.w & 0xffff0000u)};
+#pragma unroll
+                            for (int c = 0; c < C; ++c) {
+                                Z[0][c] += w0[c];
+                                A[0][c] = fmaf(w0[c], uw0[c + jj], A[0][c]);
+                                Z[1][c] += w1[c];
+                                A[1][c] = fmaf(w1[c], uw1[c + jj], A[1][c]);
+                            }
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                nbsum[0][c] += A[0][c] / Z[0][c];
+                nbsum[1][c] += A[1][c] / Z[1][c];
+            }
+        }
+        if (c0 < nx) {
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                if (r + q < ny) {
+                    const float *__restrict__ gi = g + (size_t)img * npix + (size_t)(r + q) * nx + c0;
+                    float *__restrict__ o = out + (size_t)img * npix + (size_t)(r + q) * nx + c0;
+#pragma unroll
+                    for (int c = 0; c < C; ++c)
+                        if (c0 + c < nx) {
+                            float v = fmaf(p.c_nb, nbsum[q][c], p.c_self * __ldg(gi + c));
+                            if (p.clip) v = fmaxf(v, 0.f);
+                            o[c] = v;
+                        }
+                }
+            }
+        }
+    }
 }
 
 // f = max(g, 0): the m2 = 0 case of steps 3-5.

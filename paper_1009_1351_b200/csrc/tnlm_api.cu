@@ -45,6 +45,9 @@ struct tnlm_handle {
     // tuning knobs, read once from the environment at tnlm_create (tnlm_set_option changes them later)
     long long opt_cache_mb = 16384;
     int opt_rb = 0, opt_nb = 0, opt_ns = 0;
+    int opt_apply = 1;      // 1: gj_apply2_kernel (persistent warp tasks, cp.async rings); 0: gj_apply_kernel (TMA ring)
+    int opt_depth = 0;      // gj_apply2_kernel ring depth override (0 = cost model)
+    int opt_wpc = 0;        // gj_apply2_kernel warps per CTA override (0 = cost model)
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
@@ -310,6 +313,8 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         if (ce == cudaSuccess)
             ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
                                       cudaSharedmemCarveoutMaxShared);
+        for (const void *fn : {(const void *)gj_apply2_kernel<4>, (const void *)gj_apply2_kernel<8>, (const void *)gj_apply2_kernel<16>})
+            if (ce == cudaSuccess) ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)H->apply_smem);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
     }
     H->n_sm = prop.multiProcessorCount;
@@ -699,6 +704,47 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
+    if (H->opt_apply == 1) {
+        // Persistent warp tasks (row pairs).  Launch shape by a small cost model: for every ring depth and CTA
+        // size, the resident warps W and the bytes they keep in flight bound the rate of a round at
+        // min(6.2 TB/s, in-flight / 1.5 us); tasks / W full rounds, then one round with the remaining tasks.
+        R.n_img = n_slices * H->n_phase;
+        const long long tasks = ctas * (sh.rb / 2);
+        const double task_bytes = 2.0 * H->window * H->window * 512.0;
+        int best_dp = 0, best_wpc = 0, best_per_sm = 0;
+        double best_t = 0.0;
+        for (int dp = 16; dp >= 4; dp >>= 1) {
+            if (H->opt_depth && dp != H->opt_depth) continue;                      // tuning overrides
+            const size_t wb = apply2_warp_bytes(H->window, dp);
+            for (int wpc = 8; wpc >= 2; --wpc) {
+                if (H->opt_wpc && wpc != H->opt_wpc) continue;
+                const size_t need = wpc * wb;
+                if (need > H->apply_smem) continue;
+                const int per_sm = (int)std::min<size_t>(H->smem_per_sm / (need + 1024), (size_t)(20 / wpc));   // 94 registers: 20 warps per SM
+                if (per_sm < 1) continue;
+                const long long warps = std::min<long long>((long long)H->n_sm * per_sm * wpc, tasks);
+                auto round_time = [&](long long active) {
+                    const double rate = std::min(6.2e12, (double)active * (dp - 1) * 512.0 / 1.5e-6);
+                    return (double)active * task_bytes / rate;
+                };
+                double t = (double)(tasks / warps) * round_time(warps);
+                if (tasks % warps) t += round_time(tasks % warps);
+                if (!best_dp || t < best_t * 0.999) { best_dp = dp; best_wpc = wpc; best_per_sm = per_sm; best_t = t; }
+            }
+        }
+        if (!best_dp) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+        const long long want = (tasks + best_wpc - 1) / best_wpc;
+        const unsigned grid = (unsigned)std::min<long long>((long long)H->n_sm * best_per_sm, want);
+        const size_t sm = best_wpc * apply2_warp_bytes(H->window, best_dp);
+        ProfScope ps(H, TNLM_KERNEL_APPLY, st);
+        switch (best_dp) {
+            case 16: gj_apply2_kernel<16><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
+            case 8: gj_apply2_kernel<8><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
+            default: gj_apply2_kernel<4><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
+        }
+        LAUNCHED(H);
+        return TNLM_OK;
+    }
     // ring depth: the most stages whose shared memory still leaves the last wave best filled
     const int threads = 32 * (sh.rb + 1);
     double best_eff = -1.0;
@@ -806,6 +852,9 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "sweep_rb") H->opt_rb = (int)value;
     else if (n == "sweep_nb") H->opt_nb = (int)value;
     else if (n == "apply_ns") H->opt_ns = (int)value;
+    else if (n == "apply_kernel") H->opt_apply = (int)value;
+    else if (n == "apply_depth") H->opt_depth = (int)value;
+    else if (n == "apply_wpc") H->opt_wpc = (int)value;
     else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);
     return TNLM_OK;
 }
