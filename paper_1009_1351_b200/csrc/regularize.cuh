@@ -126,6 +126,17 @@ __device__ __forceinline__ void cp_async16(void *dst, const void *src)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
+// the same with a 32-bit shared-window address (no generic -> shared conversion per copy)
+__device__ __forceinline__ void cp_async16_s(unsigned dst_s, const void *src, bool pred)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q cp.async.cg.shared.global [%0], [%1], 16;\n}" ::"r"(dst_s), "l"(src), "r"((int)pred) : "memory");
+}
+__device__ __forceinline__ uint4 lds128_s(unsigned addr_s)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr_s));
+    return v;
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
@@ -677,7 +688,7 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     extern __shared__ float4 smem4[];
     const size_t wbytes = apply2_warp_bytes(W, DEPTH);
     float *sU = reinterpret_cast<float *>(reinterpret_cast<char *>(smem4) + warp * wbytes);   // [urows][UW]
-    uint4 *ring = reinterpret_cast<uint4 *>(sU + urows * UW) + lane;                          // [DEPTH][32 lanes]
+    const unsigned ring_s = smem_u32(sU + urows * UW) + 16 * lane;                           // [DEPTH][32 lanes] x 16 B
 
     const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
     const long long n_tasks = (long long)p.n_img * tiles_per_img * npairs;
@@ -703,15 +714,17 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
             // oldest group: this side's u_j window; then pieces 0..DEPTH-2 of its weights
             stage_tile_async(sU, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, r - a, tile_c0 - a, ny, nx, 0, 1, lane);
             cp_async_commit();
+            const uint4 *__restrict__ nextp = ws;             // piece `issued` of this side
+            unsigned issued = 0;
 #pragma unroll 1
-            for (int t = 0; t < DEPTH - 1; ++t) {
-                if (t < WW) cp_async16(ring + (t % DEPTH) * 32, ws + (size_t)t * pstride);
+            for (; issued < DEPTH - 1; ++issued, nextp += pstride) {
+                cp_async16_s(ring_s + ((issued & (DEPTH - 1)) << 9), nextp, issued < (unsigned)WW);
                 cp_async_commit();
             }
             cp_async_wait<DEPTH - 1>();                       // the window has landed (every lane's part of it)
             __syncwarp();
             float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-            int t = 0;
+            unsigned t = 0;
 #pragma unroll 1
             for (int dr = 0; dr < W; ++dr) {
                 const float *__restrict__ urow0 = sU + dr * UW + C * lane;
@@ -725,11 +738,11 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
 #pragma unroll
                     for (int jj = 0; jj < 4; ++jj) {
                         if (jj < noff) {
-                            const int tn = t + DEPTH - 1;
-                            if (tn < WW) cp_async16(ring + (tn % DEPTH) * 32, ws + (size_t)tn * pstride);
+                            cp_async16_s(ring_s + ((issued & (DEPTH - 1)) << 9), nextp, issued < (unsigned)WW);
                             cp_async_commit();                // (empty groups keep the wait count uniform)
+                            ++issued; nextp += pstride;
                             cp_async_wait<DEPTH - 1>();       // piece t has landed (this lane's own 16 bytes)
-                            const uint4 wv = ring[(t % DEPTH) * 32];
+                            const uint4 wv = lds128_s(ring_s + ((t & (DEPTH - 1)) << 9));
                             ++t;
                             // bf16 -> fp32 is a 16-bit shift: low half << 16, high half masked
                             const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
