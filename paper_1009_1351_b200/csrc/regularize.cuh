@@ -346,6 +346,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
             const float4 *__restrict__ gjp = reinterpret_cast<const float4 *>(myGj + (lr0 + dr + a) * GJW) + lane + dcg;
             const float4 *__restrict__ ujp = reinterpret_cast<const float4 *>(myUj + (lr0 + dr + a) * UJW) + lane + dcg;
             const float4 *__restrict__ kp = reinterpret_cast<const float4 *>(myK) + lane;
+            uint2 held[G];                         // STORE_W: packed weights of the even row of a pair
             __nv_bfloat16 *__restrict__ witem =
                 STORE_W ? wchunk + ((size_t)(dr + a) * (2 * a + 1) + (dc0 + a)) * WSTRIDE + 8 * lane : nullptr;
 #pragma unroll
@@ -408,14 +409,21 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         }
                         ring[gg][cp][s % RING] = H2;
                     }
-                    if (STORE_W && s >= 2 * PB) {  // one predicated 8-byte store: 4 bf16 weights of row rr, offset gg
+                    if (STORE_W && s >= 2 * PB) {  // 4 bf16 weights of row rr, offset gg
                         const int rr = s - 2 * PB;
                         const __nv_bfloat162 lo = __floats2bfloat162_rn(e_[0].x, e_[0].y), hi = __floats2bfloat162_rn(e_[1].x, e_[1].y);
                         uint2 pk;
                         pk.x = *reinterpret_cast<const unsigned *>(&lo);
                         pk.y = *reinterpret_cast<const unsigned *>(&hi);
-                        if (dc0 + gg <= a)         // (rows / columns past the image edge land in chunk padding)
-                            *reinterpret_cast<uint2 *>(witem + gg * WSTRIDE + (rr >> 1) * 256 + (rr & 1) * 4) = pk;
+                        // rows 2q and 2q+1 share one 16-byte slot per lane (plane_off): the even row waits in
+                        // registers for one step, then one STG.128 per offset and row pair (8-byte stores at a
+                        // 16-byte stride cost 20 us more per cfg-2 sweep)
+                        if (rr & 1) {
+                            if (dc0 + gg <= a)     // (rows / columns past the image edge land in chunk padding)
+                                *reinterpret_cast<uint4 *>(witem + gg * WSTRIDE + (rr >> 1) * 256) = make_uint4(held[gg].x, held[gg].y, pk.x, pk.y);
+                        } else {
+                            held[gg] = pk;
+                        }
                     }
                 }
                 SW_STEP_FENCE();
