@@ -70,6 +70,38 @@ __device__ __forceinline__ float warp_sum(float v)
     return v;
 }
 
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// ---- cp.async (LDGSTS): global -> shared copies that hold no registers while in flight -----------------
+// 4-byte copy; `valid` false writes 0.0f instead (src-size 0: nothing is read).
+__device__ __forceinline__ void cp_async4_zfill(void *dst, const void *src, bool valid)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 4 : 0) : "memory");
+}
+// 16-byte copy; `valid` false writes 16 zero bytes instead
+__device__ __forceinline__ void cp_async16_zfill(void *dst, const void *src, bool valid)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(valid ? 16 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+// the same with a 32-bit shared-window address (no generic -> shared conversion per copy)
+__device__ __forceinline__ void cp_async16_s(unsigned dst_s, const void *src, bool pred)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q cp.async.cg.shared.global [%0], [%1], 16;\n}" ::"r"(dst_s), "l"(src), "r"((int)pred) : "memory");
+}
+__device__ __forceinline__ uint4 lds128_s(unsigned addr_s)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr_s));
+    return v;
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // FP32 (non-tensor) peak probe: 8 independent FFMA chains per thread, fully unrolled inner block, so the
 // loop overhead is < 2 %.  The roofline denominator of the ALU-bound kernels is measured with this on the
 // box the benchmark runs on (MEASURED_PEAKS.json has no FP32 figure).

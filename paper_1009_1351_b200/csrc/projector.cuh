@@ -7,6 +7,15 @@
 
 namespace tnlm {
 
+#ifndef TNLM_BP_UNROLL
+#define TNLM_BP_UNROLL 1
+#endif
+constexpr int BP_UNROLL = TNLM_BP_UNROLL;
+#ifndef TNLM_FP_UNROLL
+#define TNLM_FP_UNROLL 4
+#endif
+constexpr int FP_UNROLL = TNLM_FP_UNROLL;   // rows per unrolled body of the forward projector's interior loop   // candidates per unrolled body of the backprojector's inner loop
+
 enum FwdMode {
     FWD_PLAIN = 0,  // out0 = P img
     FWD_RESID = 1,  // out0 = sw*(y - P img) = r ; out1 = sw*r            (CGLS init, L109)
@@ -93,7 +102,7 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
             edge(rg.lo, rg.ilo - 1);
             float qf = (float)rg.ilo;
             const float *__restrict__ row = base + (size_t)rg.ilo * n_minor;
-#pragma unroll 4
+#pragma unroll FP_UNROLL
             for (int q = rg.ilo; q <= rg.ihi; ++q, qf += 1.0f, row += n_minor) {
                 int c0; float F1, U1;
                 ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
@@ -134,6 +143,146 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
     }
 }
 
+// The same projector with the gathers served from shared memory.  ncu on project_kernel: 51 % issue-active,
+// 19 long-scoreboard stall cycles per issue, L1TEX 60-88 % busy: two 32-lane gathers per row, each touching two or
+// three sectors of one or two lines, are what it waits for.  Here a WARP owns 32 neighbouring bins of one view and
+// walks its rows in chunks of PS_R: for a chunk it works out the columns its rays touch (lo is linear in the row,
+// so the extremes are at the chunk's ends), stages that strip (<= PS_W columns, 16-byte cp.async, zero-filled
+// outside the image so that no bounds test is left in the inner loop) in its private shared-memory slot and reads
+// both cells of every row with conflict-free LDS.  The arithmetic and its order are those of project_kernel, so
+// the result is bit-identical and P^T stays the exact transpose.  A warp whose rays are not all steep or all
+// shallow (one per view at most), an image whose rows are not 16-byte aligned, or a chunk wider than PS_W
+// columns takes the gather path.  grid = (ceil(V * ceil(B/32) / PS_WARPS), S*N); block = 32 * PS_WARPS.
+constexpr int PS_R = 16;        // rows per staged chunk
+constexpr int PS_W = 64;        // columns per strip row
+constexpr int PS_WARPS = 8;
+
+template <int MODE>
+__global__ void __launch_bounds__(32 * PS_WARPS)
+project_strip_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
+                     const float *__restrict__ img, const float *__restrict__ imgT, const float *__restrict__ y,
+                     const float *__restrict__ sw_, float *__restrict__ out0, float *__restrict__ out1,
+                     double *__restrict__ red)
+{
+    __shared__ __align__(16) float strip_all[PS_WARPS][PS_R * PS_W];
+    const int prob = blockIdx.y;                 // slice*N + phase
+    const int phase = prob % G.n_phase;
+    const int V = G.n_views, B = G.n_bins, nray = V * B;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int WB = (B + 31) >> 5;                // warp tasks per view
+    const int task = blockIdx.x * PS_WARPS + warp;
+    const int v = task / WB, k = (task - v * WB) * 32 + lane;
+    const bool valid = (v < V) && (k < B);
+    const int ray = v * B + k;
+    float *__restrict__ strip = strip_all[warp];
+    float qq = 0.f;
+    RayEntry e = {0.f, 0.f, 1.f, 1.f};
+    RayRange rg = {1, 0, 1, 0};
+    if (valid) {
+        e = tab[(size_t)phase * nray + ray];
+        rg = rng[(size_t)phase * nray + ray];
+    }
+    const bool active = valid && rg.hi >= rg.lo;
+    const bool steep = e.len > 0.f;
+    const unsigned m_act = __ballot_sync(0xffffffffu, active), m_steep = __ballot_sync(0xffffffffu, active && steep);
+    const bool uniform = (m_steep == m_act) || (m_steep == 0u);
+    const bool steep_w = m_steep != 0u;
+    const int n_minor_w = steep_w ? G.nx : G.ny, n_major_w = steep_w ? G.ny : G.nx;
+    const float *__restrict__ base_w = (steep_w ? img : imgT) + (size_t)prob * G.nx * G.ny;
+    const bool can_stage = uniform && ((n_minor_w & 3) == 0) && ((reinterpret_cast<uintptr_t>(base_w) & 15) == 0);
+    float acc0 = 0.f, acc1 = 0.f;                // sums of fraction x pixel value; x alen once at the end
+    // rows [q0, q1] of this lane's ray by gathers from global memory (bounds-tested)
+    auto gather = [&](int q0, int q1) {
+        const int n_minor = steep ? G.nx : G.ny;
+        const float *__restrict__ row = (steep ? img : imgT) + (size_t)prob * G.nx * G.ny + (size_t)q0 * n_minor;
+        float qf = (float)q0;
+        for (int q = q0; q <= q1; ++q, qf += 1.0f, row += n_minor) {
+            int c0; float F1, U1;
+            ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+            if ((unsigned)c0 < (unsigned)n_minor) acc0 = fmaf(F1, __ldg(row + c0), acc0);
+            if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1 = fmaf(U1, __ldg(row + c0 + 1), acc1);
+        }
+    };
+    if (!can_stage) {
+        if (active) gather(rg.lo, rg.hi);
+    } else if (m_act) {
+        const int q_begin = __reduce_min_sync(0xffffffffu, active ? (int)rg.lo : 0x7fffffff);
+        const int q_end = __reduce_max_sync(0xffffffffu, active ? (int)rg.hi : -1);
+        for (int qa = q_begin; qa <= q_end; qa += PS_R) {
+            const int qb = min(qa + PS_R - 1, q_end);
+            const int my_a = max(qa, (int)rg.lo), my_b = min(qb, (int)rg.hi);
+            const bool has = active && my_a <= my_b;
+            // columns this lane touches in the chunk: lo is linear in the row, extremes at its two ends
+            const float la = ray_lo(e.plo, e.m, (float)my_a), lb = ray_lo(e.plo, e.m, (float)my_b);
+            const int cl = __float_as_int(__fadd_rd(fminf(la, lb), FLOOR_MAGIC)) - FLOOR_MAGIC_BITS;
+            const int ch = __float_as_int(__fadd_rd(fmaxf(la, lb), FLOOR_MAGIC)) - FLOOR_MAGIC_BITS + 1;
+            const int cmin = __reduce_min_sync(0xffffffffu, has ? cl : 0x7fffffff);
+            const int cmax = __reduce_max_sync(0xffffffffu, has ? ch : (int)0x80000000);
+            if (cmin > cmax) continue;                       // no lane has a row in this chunk
+            const int c_al = cmin & ~3;                      // (two's complement: rounds towards -inf)
+            const int ngrp = ((cmax - c_al) >> 2) + 1;       // 16-byte groups per strip row
+            if (ngrp * 4 > PS_W) {                           // too wide for the slot (a very oblique geometry)
+                if (has) gather(my_a, my_b);
+                continue;
+            }
+            __syncwarp();                                    // the previous chunk is no longer read
+            {   // lanes 0-15 stage the groups of one row, lanes 16-31 those of the next
+                const int gi = lane & 15, c = c_al + 4 * gi;
+                const bool cin = gi < ngrp && (unsigned)c < (unsigned)n_minor_w;
+                for (int rr = lane >> 4; qa + rr <= qb; rr += 2) {
+                    const int q = qa + rr;
+                    const bool in = cin && (unsigned)q < (unsigned)n_major_w;
+                    if (gi < ngrp)
+                        cp_async16_zfill(strip + rr * PS_W + 4 * gi, base_w + (in ? (size_t)q * n_minor_w + c : 0), in);
+                }
+            }
+            cp_async_commit();
+            cp_async_wait<0>();
+            __syncwarp();
+            if (has) {
+                const float *__restrict__ srow = strip + (my_a - qa) * PS_W - c_al;
+                float qf = (float)my_a;
+#pragma unroll 4
+                for (int q = my_a; q <= my_b; ++q, qf += 1.0f, srow += PS_W) {
+                    int c0; float F1, U1;
+                    ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+                    acc0 = fmaf(F1, srow[c0], acc0);
+                    acc1 = fmaf(U1, srow[c0 + 1], acc1);
+                }
+            }
+        }
+    }
+    if (valid) {
+        const float p = __fmul_rn(fabsf(e.len), acc0 + acc1);
+        const size_t o = (size_t)prob * nray + ray;
+        if (MODE == FWD_PLAIN) {
+            out0[o] = p;
+        } else {
+            const float sw = sw_ ? sw_[o] : 1.0f;
+            if (MODE == FWD_RESID) {
+                const float r = sw * (y[o] - p);
+                out0[o] = r;
+                out1[o] = sw * r;
+            } else {
+                const float q = sw * p;
+                out0[o] = q;
+                qq = q * q;
+            }
+        }
+    }
+    if (MODE == FWD_SCALE) {
+        __shared__ float part[PS_WARPS];
+        qq = warp_sum(qq);
+        if (lane == 0) part[warp] = qq;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            float vv = threadIdx.x < PS_WARPS ? part[threadIdx.x] : 0.f;
+            vv = warp_sum(vv);
+            if (threadIdx.x == 0) atomicAdd(red + prob, (double)vv);
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------- adjoint
 // grid = (ceil(nx/16), ceil(ny/32), S*N); block = 128 threads.  One thread per 2 x 2 pixel block
 // (rows r0, r0+1, columns c0, c0+1; a warp covers 16 x 8 pixels), loop over the views of its
@@ -162,9 +311,11 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
         const float Y = ((float)r0 + 0.5f - 0.5f * (float)(G.ny - 1)) * G.pix;
         const float rf = (float)r0, cf = (float)c0, dcr = cf - rf, rfm1 = rf - 1.0f;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
-        const float4 *__restrict__ tb = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
-        const float *__restrict__ sg = sino + (size_t)prob * V * B;
-        for (int v = 0; v < V; ++v, tb += B, sg += B) {
+        const float4 *__restrict__ tb0 = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
+        const float *__restrict__ sg0 = sino + (size_t)prob * V * B;
+        const float hw2 = 2.0f * G.hw_scale;
+        int vB = 0;                                          // v * B: 32-bit offsets into the phase's table and sinogram
+        for (int v = 0; v < V; ++v, vB += B) {
             const float4 vw = __ldg(vt + v);                 // sx, sy, cos th, sin th
             const float px = X - vw.x, py = Y - vw.y;
             const float dot = -(vw.z * px + vw.w * py);      // along the central ray (> 0)
@@ -174,16 +325,17 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             const float t = crs * rdot;
             const float kc = fmaf(POLY ? fan_angle_poly(t) : atanf(t), G.sdd_over_pitch, G.bin_centre);
             // the block's angular half-width is <= (pix*sqrt 2)/distance <= (pix*sqrt 2)/dot
-            const float hw = fmaf(2.0f * G.hw_scale, rdot, 0.05f);
+            const float hw = fmaf(hw2, rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
-            const float4 *__restrict__ tbk = tb + k_lo;
-            const float *__restrict__ sgk = sg + k_lo;
+            const float4 *__restrict__ tbk = tb0 + (vB + k_lo);
+            const float *__restrict__ sgk = sg0 + (vB + k_lo);
             // Membership and lengths by FP32-pipe arithmetic only: st = 1 for a steep ray, 0 for a shallow one;
             // evaluation j is in row r0+j (steep) or column c0+j (shallow); the block's two pixels in that line
             // sit at minor-axis indices cA and cA+1 (cA = c0 steep, r0 shallow) and get
             // alen * (F(cA+1) - F(cA)) and alen * (F(cA+2) - F(cA+1)), F = ray_cum (common.cuh): zero for cells
             // the ray misses, and bit for bit the forward projector's entry for the cells it touches.
+#pragma unroll BP_UNROLL
             for (int n = k_hi - k_lo; n >= 0; --n, ++tbk, ++sgk) {
                 const float4 e4 = __ldg(tbk);                // plo, m, len (sign = steep), inva
                 const float sv = __ldg(sgk);
@@ -195,7 +347,7 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
                 float dA[2], dB[2];
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const float lo = ray_lo(e4.x, e4.y, qf + (float)j);
+                    const float lo = ray_lo(e4.x, e4.y, j ? qf + 1.0f : qf);
                     const float G0 = ray_cum(me0, lo, e4.w), G1 = ray_cum(me1, lo, e4.w), G2 = ray_cum(me2, lo, e4.w);
                     dA[j] = __fsub_rn(G1, G0);
                     dB[j] = __fsub_rn(G2, G1);
