@@ -313,7 +313,6 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
         const float4 *__restrict__ vt = views + (size_t)phase * V;
         const float4 *__restrict__ tb0 = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg0 = sino + (size_t)prob * V * B;
-        const float hw2 = 2.0f * G.hw_scale;
         int vB = 0;                                          // v * B: 32-bit offsets into the phase's table and sinogram
         for (int v = 0; v < V; ++v, vB += B) {
             const float4 vw = __ldg(vt + v);                 // sx, sy, cos th, sin th
@@ -324,8 +323,10 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rdot) : "f"(dot));
             const float t = crs * rdot;
             const float kc = fmaf(POLY ? fan_angle_poly(t) : atanf(t), G.sdd_over_pitch, G.bin_centre);
-            // the block's angular half-width is <= (pix*sqrt 2)/distance <= (pix*sqrt 2)/dot
-            const float hw = fmaf(hw2, rdot, 0.05f);
+            // a ray crosses the 2 x 2 block (half-side pix) iff it passes within pix*(|nx|+|ny|) of its centre, n the
+            // ray's unit normal ~ (-py, px)/d: angular half-width pix*(|px|+|py|)/d^2 <= pix*(|px|+|py|)/dot^2
+            // (hw_scale carries pix, bins per radian and 2 % for the second-order terms), + 0.05 bin of rounding
+            const float hw = fmaf(G.hw_scale * (fabsf(px) + fabsf(py)), rdot * rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const float4 *__restrict__ tbk = tb0 + (vB + k_lo);

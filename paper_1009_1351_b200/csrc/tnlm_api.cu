@@ -338,7 +338,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
             const double rmax = std::sqrt(hx * hx + hy * hy) + g.pixel_mm;
             H->fan_poly = rmax / std::sqrt(std::fmax(g.sid_mm * g.sid_mm - rmax * rmax, 1e-30)) < 0.95;
         }
-        G.hw_scale = (float)(1.02 * g.pixel_mm * 0.70710678118654752 * g.sdd_mm / g.bin_pitch_mm);
+        G.hw_scale = (float)(1.02 * g.pixel_mm * g.sdd_mm / g.bin_pitch_mm);
         std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views;
         build_tables(g, nx, ny, n_phase, tab, rng, views);
         bool ok = cudaMalloc(&H->d_tab, tab.size() * sizeof(RayEntry)) == cudaSuccess &&
