@@ -88,7 +88,7 @@ def projector_work(cfg, n_slices):
 class ClockSampler:
     """Samples SM clock and throttle reasons (NVML) in a thread while the timed region runs."""
 
-    def __init__(self, torch_device_index, period=0.05):
+    def __init__(self, torch_device_index, period=0.002):
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
         self._thr = None
