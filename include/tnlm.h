@@ -54,7 +54,11 @@
  *   from the environment ONCE at tnlm_create and changed later with tnlm_set_option:
  *   weight_cache_mb / TNLM_WEIGHT_CACHE_MB (default 16384; larger needs, or 0, make every sweep
  *   recompute the weights in fp32), sweep_rb, sweep_nb / TNLM_SWEEP_SHAPE="rb,nb" and
- *   apply_ns / TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).
+ *   apply_ns / TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).  Options without an
+ *   environment variable (kernel variants kept for comparison; results are bit-identical either way):
+ *   apply_kernel (1 = persistent warp-task stored-weight sweep, the default; 0 = one CTA per band with a TMA
+ *   ring), apply_depth, apply_wpc (ring depth and warps per CTA of the former; 0 = cost model),
+ *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers).
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
@@ -153,7 +157,8 @@ const char *tnlm_last_error(const tnlm_handle *handle);
 int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_entry_points);
 
 /* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
- * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns"; 0 restores the heuristic for the last three. */
+ * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns", "apply_kernel", "apply_depth", "apply_wpc",
+ * "project_kernel"; 0 restores the heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
 int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
 
 /* The CUDA device ordinal the handle was created on (-1 for a NULL handle). */
