@@ -860,15 +860,18 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     H->err.clear();
     if (!name) return fail(H, TNLM_INVALID_ARG, "option name is NULL");
     const std::string n(name);
+    auto in = [&](long long lo, long long hi) { return value >= lo && value <= hi; };
+    bool ok = true;
     if (n == "weight_cache_mb") H->opt_cache_mb = value;
     else if (n == "sweep_rb") H->opt_rb = (int)value;
     else if (n == "sweep_nb") H->opt_nb = (int)value;
-    else if (n == "apply_ns") H->opt_ns = (int)value;
-    else if (n == "apply_kernel") H->opt_apply = (int)value;
-    else if (n == "project_kernel") H->opt_project = (int)value;
-    else if (n == "apply_depth") H->opt_depth = (int)value;
-    else if (n == "apply_wpc") H->opt_wpc = (int)value;
+    else if (n == "apply_ns") { if ((ok = in(0, AP_NS_MAX))) H->opt_ns = (int)value; }
+    else if (n == "apply_kernel") { if ((ok = in(0, 1))) H->opt_apply = (int)value; }
+    else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
+    else if (n == "apply_depth") { if ((ok = (value == 0 || value == 4 || value == 8 || value == 16))) H->opt_depth = (int)value; }
+    else if (n == "apply_wpc") { if ((ok = (value == 0 || in(2, 8)))) H->opt_wpc = (int)value; }
     else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);
+    if (!ok) return fail(H, TNLM_INVALID_ARG, "value out of range for option " + n);
     return TNLM_OK;
 }
 
