@@ -3,12 +3,14 @@
 // Both kernels evaluate tnlm::ray_cum on the same RayEntry table, so every matrix entry
 // len(ray ∩ pixel) is bit-identical on the two sides and P^T is the exact transpose of P (common.cuh).
 #pragma once
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace tnlm {
 
 #ifndef TNLM_BP_UNROLL
-#define TNLM_BP_UNROLL 1
+#define TNLM_BP_UNROLL 2
 #endif
 constexpr int BP_UNROLL = TNLM_BP_UNROLL;
 #ifndef TNLM_FP_UNROLL
@@ -295,7 +297,8 @@ project_strip_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *_
 template <bool POLY>
 __global__ void __launch_bounds__(128)
 backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__restrict__ views,
-                   const float *__restrict__ sino, float *__restrict__ out, double *__restrict__ red)
+                   const int4 *__restrict__ split, const float *__restrict__ sino, float *__restrict__ out,
+                   double *__restrict__ red)
 {
     const int prob = blockIdx.z;
     const int phase = prob % G.n_phase;
@@ -309,13 +312,41 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
         // block centre
         const float X = ((float)c0 + 0.5f - 0.5f * (float)(G.nx - 1)) * G.pix;
         const float Y = ((float)r0 + 0.5f - 0.5f * (float)(G.ny - 1)) * G.pix;
-        const float rf = (float)r0, cf = (float)c0, dcr = cf - rf, rfm1 = rf - 1.0f;
+        const float rf = (float)r0, cf = (float)c0;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
+        const int4 *__restrict__ spl = split + (size_t)phase * V;
         const float4 *__restrict__ tb0 = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg0 = sino + (size_t)prob * V * B;
-        int vB = 0;                                          // v * B: 32-bit offsets into the phase's table and sinogram
+        // Candidates kb0..kb1 (offsets into the phase's table / the sinogram) of ONE class: steep rays are evaluated
+        // in rows r0, r0+1 and the block's two pixels of a row sit at minor-axis indices c0, c0+1; shallow rays in
+        // columns c0, c0+1 with minor-axis indices r0, r0+1.  The two pixels of line j get alen * (F(cA+1) - F(cA))
+        // and alen * (F(cA+2) - F(cA+1)), F = ray_cum (common.cuh): zero for cells the ray misses, and bit for bit
+        // the forward projector's entry for the cells it touches -- no membership test anywhere.
+        auto run = [&](auto steep_c, int kb0, int kb1) {
+            constexpr bool STEEP = decltype(steep_c)::value;
+            const float q0 = STEEP ? rf : cf, q1 = q0 + 1.0f;
+            const float m0 = (STEEP ? cf : rf) - 1.0f, m1 = m0 + 1.0f, m2 = m0 + 2.0f;
+            const float4 *__restrict__ tp = tb0 + kb0;
+            const float *__restrict__ sp = sg0 + kb0;
+#pragma unroll BP_UNROLL
+            for (int n = kb1 - kb0; n >= 0; --n, ++tp, ++sp) {
+                const float4 e4 = __ldg(tp);                 // plo, m, len (sign = steep), inva
+                const float asv = __fmul_rn(fabsf(e4.z), __ldg(sp));
+                const float lo0 = ray_lo(e4.x, e4.y, q0), lo1 = ray_lo(e4.x, e4.y, q1);
+                const float G00 = ray_cum(m0, lo0, e4.w), G01 = ray_cum(m1, lo0, e4.w), G02 = ray_cum(m2, lo0, e4.w);
+                const float G10 = ray_cum(m0, lo1, e4.w), G11 = ray_cum(m1, lo1, e4.w), G12 = ray_cum(m2, lo1, e4.w);
+                const float dA0 = __fsub_rn(G01, G00), dB0 = __fsub_rn(G02, G01);
+                const float dA1 = __fsub_rn(G11, G10), dB1 = __fsub_rn(G12, G11);
+                a00 = __fmaf_rn(asv, dA0, a00);
+                a11 = __fmaf_rn(asv, dB1, a11);
+                a01 = __fmaf_rn(asv, STEEP ? dB0 : dA1, a01);
+                a10 = __fmaf_rn(asv, STEEP ? dA1 : dB0, a10);
+            }
+        };
+        int vB = 0;                                          // v * B
         for (int v = 0; v < V; ++v, vB += B) {
             const float4 vw = __ldg(vt + v);                 // sx, sy, cos th, sin th
+            const int4 sp = __ldg(spl + v);                  // bins [0, sp.x) and [sp.y, B) are of class sp.z (1 = steep), [sp.x, sp.y) of the other
             const float px = X - vw.x, py = Y - vw.y;
             const float dot = -(vw.z * px + vw.w * py);      // along the central ray (> 0)
             const float crs = vw.w * px - vw.z * py;         // ccw from the central ray
@@ -329,35 +360,18 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             const float hw = fmaf(G.hw_scale * (fabsf(px) + fabsf(py)), rdot * rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
-            const float4 *__restrict__ tbk = tb0 + (vB + k_lo);
-            const float *__restrict__ sgk = sg0 + (vB + k_lo);
-            // Membership and lengths by FP32-pipe arithmetic only: st = 1 for a steep ray, 0 for a shallow one;
-            // evaluation j is in row r0+j (steep) or column c0+j (shallow); the block's two pixels in that line
-            // sit at minor-axis indices cA and cA+1 (cA = c0 steep, r0 shallow) and get
-            // alen * (F(cA+1) - F(cA)) and alen * (F(cA+2) - F(cA+1)), F = ray_cum (common.cuh): zero for cells
-            // the ray misses, and bit for bit the forward projector's entry for the cells it touches.
-#pragma unroll BP_UNROLL
-            for (int n = k_hi - k_lo; n >= 0; --n, ++tbk, ++sgk) {
-                const float4 e4 = __ldg(tbk);                // plo, m, len (sign = steep), inva
-                const float sv = __ldg(sgk);
-                const float st = __saturatef(e4.z * 1.0e30f);
-                const float qf = __fmaf_rn(st, -dcr, cf);    // rf (steep) or cf (shallow), exactly
-                const float me0 = __fmaf_rn(st, dcr, rfm1);  // cA - 1: cf - 1 (steep) or rf - 1 (shallow), exactly
-                const float me1 = me0 + 1.0f, me2 = me0 + 2.0f;
-                const float asv = __fmul_rn(fabsf(e4.z), sv);
-                float dA[2], dB[2];
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const float lo = ray_lo(e4.x, e4.y, j ? qf + 1.0f : qf);
-                    const float G0 = ray_cum(me0, lo, e4.w), G1 = ray_cum(me1, lo, e4.w), G2 = ray_cum(me2, lo, e4.w);
-                    dA[j] = __fsub_rn(G1, G0);
-                    dB[j] = __fsub_rn(G2, G1);
-                }
-                const bool steep = e4.z > 0.f;
-                a00 = __fmaf_rn(asv, dA[0], a00);
-                a11 = __fmaf_rn(asv, dB[1], a11);
-                a01 = __fmaf_rn(asv, steep ? dB[0] : dA[1], a01);
-                a10 = __fmaf_rn(asv, steep ? dA[1] : dB[0], a10);
+            // the steep / shallow classes are contiguous runs of the bin index (a fan narrower than 90 degrees crosses a
+            // 45-degree direction at most once, one narrower than 180 degrees at most twice): one specialised loop per
+            // run, nearly always only one of them is non-empty
+            const int a1 = min(k_hi, sp.x - 1), b0 = max(k_lo, sp.x), b1 = min(k_hi, sp.y - 1), c0k = max(k_lo, sp.y);
+            if (sp.z) {
+                run(std::true_type{}, vB + k_lo, vB + a1);
+                run(std::false_type{}, vB + b0, vB + b1);
+                run(std::true_type{}, vB + c0k, vB + k_hi);
+            } else {
+                run(std::false_type{}, vB + k_lo, vB + a1);
+                run(std::true_type{}, vB + b0, vB + b1);
+                run(std::false_type{}, vB + c0k, vB + k_hi);
             }
         }
         float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + (size_t)r0 * G.nx + c0;

@@ -53,6 +53,7 @@ struct tnlm_handle {
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
     float4 *d_views = nullptr;
+    int4 *d_split = nullptr;         // per (phase, view): the runs of steep / shallow bins (backproject_kernel)
     // FBP initialisation (fbp.cuh): ramp filter table, cosine weights, view weights; filtered sinograms
     double *d_fbp_g = nullptr;
     float *d_fbp_cosw = nullptr, *d_fbp_wv = nullptr;
@@ -132,13 +133,16 @@ extern "C" long long tnlm_launch_count(const tnlm_handle *h) { return h ? h->lau
 // Ray (phase i, view v, bin k) in grid units (pixel c covers [c, c+1) in xi, row r in eta):
 // source (xs, es), unit direction (dx, dy).  Steep (|dy| >= |dx|): xi(eta) = p0 + m*eta with
 // m = dx/dy, p0 = xs - m*es, length per full row = pix/|dy|.  Shallow: roles swapped.
-static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, std::vector<RayEntry> &tab,
-                         std::vector<RayRange> &rng, std::vector<float4> &views)
+// Returns false if some view has more than three runs of steep / shallow bins (a fan of 180 degrees or more).
+static bool build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, std::vector<RayEntry> &tab,
+                         std::vector<RayRange> &rng, std::vector<float4> &views, std::vector<int4> &split)
 {
     const int V = g.n_views, B = g.n_bins;
     tab.resize((size_t)n_phase * V * B);
     rng.resize(tab.size());
     views.resize((size_t)n_phase * V);
+    split.resize((size_t)n_phase * V);
+    bool ok = true;
     for (int i = 0; i < n_phase; ++i)
         for (int v = 0; v < V; ++v) {
             const double th = g.angles_rad[(size_t)i * V + v];
@@ -189,7 +193,19 @@ static void build_tables(const tnlm_geometry &g, int nx, int ny, int n_phase, st
                 tab[((size_t)i * V + v) * B + k] = e;
                 rng[((size_t)i * V + v) * B + k] = r;
             }
+            // runs of steep (len > 0) / shallow bins of this view: [0, s1) and [s2, B) of class c0, [s1, s2) of the other
+            const RayEntry *row = &tab[((size_t)i * V + v) * B];
+            const int c0 = row[0].len > 0.f ? 1 : 0;
+            int s1 = B, s2 = B, runs = 1;
+            for (int k = 1; k < B; ++k)
+                if ((row[k].len > 0.f) != (row[k - 1].len > 0.f)) {
+                    ++runs;
+                    if (runs == 2) s1 = k; else if (runs == 3) s2 = k;
+                }
+            if (runs > 3) ok = false;
+            split[(size_t)i * V + v] = make_int4(s1, s2, c0, 0);
         }
+    return ok;
 }
 
 // Every compiled (PB, RB) of gj_sweep_kernel, with nb in {4, 2, 1}, that fits one CTA's shared
@@ -339,9 +355,14 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
             H->fan_poly = rmax / std::sqrt(std::fmax(g.sid_mm * g.sid_mm - rmax * rmax, 1e-30)) < 0.95;
         }
         G.hw_scale = (float)(1.02 * g.pixel_mm * g.sdd_mm / g.bin_pitch_mm);
-        std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views;
-        build_tables(g, nx, ny, n_phase, tab, rng, views);
-        bool ok = cudaMalloc(&H->d_tab, tab.size() * sizeof(RayEntry)) == cudaSuccess &&
+        std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views; std::vector<int4> split;
+        if (!build_tables(g, nx, ny, n_phase, tab, rng, views, split)) {
+            tnlm_destroy(H);
+            return fail(nullptr, TNLM_UNSUPPORTED, "geometry: a view's rays change between steep and shallow more than twice (fan of 180 degrees or more)");
+        }
+        bool ok = cudaMalloc(&H->d_split, split.size() * sizeof(int4)) == cudaSuccess &&
+                  cudaMemcpy(H->d_split, split.data(), split.size() * sizeof(int4), cudaMemcpyHostToDevice) == cudaSuccess &&
+                  cudaMalloc(&H->d_tab, tab.size() * sizeof(RayEntry)) == cudaSuccess &&
                   cudaMalloc(&H->d_rng, rng.size() * sizeof(RayRange)) == cudaSuccess &&
                   cudaMalloc(&H->d_views, views.size() * sizeof(float4)) == cudaSuccess;
         if (ok) ok = cudaMemcpy(H->d_tab, tab.data(), tab.size() * sizeof(RayEntry), cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -414,6 +435,7 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     if (H->d_tab) cudaFree(H->d_tab);
     if (H->d_rng) cudaFree(H->d_rng);
     if (H->d_views) cudaFree(H->d_views);
+    if (H->d_split) cudaFree(H->d_split);
     delete H;
     return TNLM_OK;
 }
@@ -523,8 +545,8 @@ static int launch_backproject(tnlm_handle *H, const float *sino, float *img, dou
 {
     ProfScope ps(H, TNLM_KERNEL_BACKPROJECT, st);
     dim3 grid((H->nx + 15) / 16, (H->ny + 31) / 32, n_slices * H->n_phase);
-    if (H->fan_poly) backproject_kernel<true><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
-    else backproject_kernel<false><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, sino, img, red);
+    if (H->fan_poly) backproject_kernel<true><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red);
+    else backproject_kernel<false><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red);
     LAUNCHED(H);
     return TNLM_OK;
 }
