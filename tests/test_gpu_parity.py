@@ -182,13 +182,16 @@ def test_strip_and_gather_forward_projectors_are_bit_identical(T, cfg):
     assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
 
 
-def test_backprojector_candidate_range_misses_no_ray(T):
+@pytest.mark.parametrize("B,V", [(120, 16), (200, 9)], ids=["fan76", "fan127"])
+def test_backprojector_candidate_range_misses_no_ray(T, B, V):
     # The gather's candidate bins per (2 x 2 block, view) are a conservative range around the block centre's fan
     # angle; a range one bin too narrow would drop matrix entries silently.  On a mid-size geometry with a wide fan and
     # a near source (large, direction-dependent angular footprints) every entry of P^T must equal P's, bit for bit:
     # checked on unit sinograms of sampled rays against the columns the forward projector produces.
     torch, tn = T
-    cfg = workloads.Config("wide", L=40, N=1, V=16, B=120, pitch=1.0, sid=45.0, sdd=90.0, window=3, patch=3)
+    # (B = 200: a 127-degree fan, so a view's bins change between steep and shallow twice: three runs in the
+    # backprojector's per-view run table)
+    cfg = workloads.Config("wide", L=40, N=1, V=V, B=B, pitch=1.0, sid=45.0, sdd=90.0, window=3, patch=3)
     h, og = handles(tn, cfg)
     npx, nr = cfg.L * cfg.L, cfg.V * cfg.B
     eye = torch.eye(npx, device="cuda").view(npx, 1, cfg.L, cfg.L)
