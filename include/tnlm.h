@@ -58,7 +58,13 @@
  *   environment variable (kernel variants kept for comparison; results are bit-identical either way):
  *   apply_kernel (1 = persistent warp-task stored-weight sweep, the default; 0 = one CTA per band with a TMA
  *   ring), apply_depth, apply_wpc (ring depth and warps per CTA of the former; 0 = cost model),
- *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers).
+ *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers),
+ *   apply_snake (1, the default: successive stored-weight sweeps deal their tasks in opposite orders, so a sweep
+ *   starts on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored
+ *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first),
+ *   backproject_group (8, the default; 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
+ *   share the geometry (nothing couples them, L77), so one thread of a projector serves up to that many slices
+ *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change.
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
@@ -158,7 +164,8 @@ int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_ent
 
 /* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
  * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns", "apply_kernel", "apply_depth", "apply_wpc",
- * "project_kernel"; 0 restores the heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
+ * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "backproject_group"; 0 restores the
+ * heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
 int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
 
 /* The CUDA device ordinal the handle was created on (-1 for a NULL handle). */

@@ -92,6 +92,28 @@ __device__ __forceinline__ void cp_async16_s(unsigned dst_s, const void *src, bo
 {
     asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q cp.async.cg.shared.global [%0], [%1], 16;\n}" ::"r"(dst_s), "l"(src), "r"((int)pred) : "memory");
 }
+// L2 eviction-priority policies (createpolicy) and accesses that carry one: the part of a re-read stream that
+// fits in L2 is marked evict_last and stays there between kernels, the rest is marked evict_first.
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void cp_async16_s_hint(unsigned dst_s, const void *src, bool pred, uint64_t pol)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %3;\n}" ::"r"(dst_s), "l"(src), "r"((int)pred), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void stg128_hint(void *dst, const uint4 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(dst), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol) : "memory");
+}
 __device__ __forceinline__ uint4 lds128_s(unsigned addr_s)
 {
     uint4 v;

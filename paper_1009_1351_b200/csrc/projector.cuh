@@ -69,23 +69,33 @@ transpose_kernel(const float *__restrict__ img, float *__restrict__ imgT, int nx
     }
 }
 
-template <int MODE>
+// NS slices of the batch share one thread: the slices of a batch have the same geometry (nothing
+// couples them, and the gantry does not know about slices), so the walk of a ray -- ray_frac per row -- is done
+// once and only the two loads and two FMAs per row are per slice (6 + 4 NS instructions per row instead of 10 NS,
+// and 2 NS independent gathers in flight).  Per slice the arithmetic and its order are those of NS = 1.
+// grid = (ceil(V*B/256), groups*N), group g = slices slice0 + g*NS .. + NS-1.
+template <int MODE, int NS>
 __global__ void __launch_bounds__(256)
 project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
                const float *__restrict__ img, const float *__restrict__ imgT, const float *__restrict__ y,
                const float *__restrict__ sw_, float *__restrict__ out0, float *__restrict__ out1,
-               double *__restrict__ red)
+               double *__restrict__ red, int slice0)
 {
-    const int prob = blockIdx.y;                 // slice*N + phase
-    const int phase = prob % G.n_phase;
+    const int phase = blockIdx.y % G.n_phase;
+    const int prob = (slice0 + (blockIdx.y / G.n_phase) * NS) * G.n_phase + phase;   // slice*N + phase of the group's first slice
     const int nray = G.n_views * G.n_bins;
+    const size_t img_stride = (size_t)G.n_phase * G.nx * G.ny, sino_stride = (size_t)G.n_phase * nray;   // per slice
     const int ray = blockIdx.x * blockDim.x + threadIdx.x;
-    float qq = 0.f;
+    float qq[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) qq[s] = 0.f;
     if (ray < nray) {
         const RayEntry e = tab[(size_t)phase * nray + ray];
         const RayRange rg = rng[(size_t)phase * nray + ray];
         const float alen = fabsf(e.len);
-        float acc0 = 0.f, acc1 = 0.f;                            // sums of fraction x pixel value; x alen once at the end
+        float acc0[NS], acc1[NS];                              // sums of fraction x pixel value; x alen once at the end
+#pragma unroll
+        for (int s = 0; s < NS; ++s) { acc0[s] = 0.f; acc1[s] = 0.f; }
         // steep rays walk the rows of the image, shallow rays the rows of the transposed image
         const bool steep = e.len > 0.f;
         const int n_minor = steep ? G.nx : G.ny;             // length of a walked row
@@ -96,51 +106,65 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
             for (int q = q0; q <= q1; ++q, qf += 1.0f, row += n_minor) {
                 int c0; float F1, U1;
                 ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
-                if ((unsigned)c0 < (unsigned)n_minor) acc0 = fmaf(F1, __ldg(row + c0), acc0);
-                if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1 = fmaf(U1, __ldg(row + c0 + 1), acc1);
+#pragma unroll
+                for (int s = 0; s < NS; ++s) {
+                    if ((unsigned)c0 < (unsigned)n_minor) acc0[s] = fmaf(F1, __ldg(row + s * img_stride + c0), acc0[s]);
+                    if ((unsigned)(c0 + 1) < (unsigned)n_minor) acc1[s] = fmaf(U1, __ldg(row + s * img_stride + c0 + 1), acc1[s]);
+                }
             }
         };
         if (rg.ihi >= rg.ilo) {
             edge(rg.lo, rg.ilo - 1);
             float qf = (float)rg.ilo;
             const float *__restrict__ row = base + (size_t)rg.ilo * n_minor;
-#pragma unroll FP_UNROLL
+#pragma unroll (NS == 1 ? FP_UNROLL : (NS == 2 ? 2 : 1))
             for (int q = rg.ilo; q <= rg.ihi; ++q, qf += 1.0f, row += n_minor) {
                 int c0; float F1, U1;
                 ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
-                acc0 = fmaf(F1, __ldg(row + c0), acc0);
-                acc1 = fmaf(U1, __ldg(row + c0 + 1), acc1);
+                const float *__restrict__ cell = row + c0;
+#pragma unroll
+                for (int s = 0; s < NS; ++s) {
+                    acc0[s] = fmaf(F1, __ldg(cell + s * img_stride), acc0[s]);
+                    acc1[s] = fmaf(U1, __ldg(cell + s * img_stride + 1), acc1[s]);
+                }
             }
             edge(rg.ihi + 1, rg.hi);
         } else {
             edge(rg.lo, rg.hi);
         }
-        const float p = __fmul_rn(alen, acc0 + acc1);
-        const size_t o = (size_t)prob * nray + ray;
-        if (MODE == FWD_PLAIN) {
-            out0[o] = p;
-        } else {
-            const float sw = sw_ ? sw_[o] : 1.0f;
-            if (MODE == FWD_RESID) {
-                const float r = sw * (y[o] - p);
-                out0[o] = r;
-                out1[o] = sw * r;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float p = __fmul_rn(alen, acc0[s] + acc1[s]);
+            const size_t o = (size_t)prob * nray + s * sino_stride + ray;
+            if (MODE == FWD_PLAIN) {
+                out0[o] = p;
             } else {
-                const float q = sw * p;
-                out0[o] = q;
-                qq = q * q;
+                const float sw = sw_ ? sw_[o] : 1.0f;
+                if (MODE == FWD_RESID) {
+                    const float r = sw * (y[o] - p);
+                    out0[o] = r;
+                    out1[o] = sw * r;
+                } else {
+                    const float q = sw * p;
+                    out0[o] = q;
+                    qq[s] = q * q;
+                }
             }
         }
     }
     if (MODE == FWD_SCALE) {
-        __shared__ float part[8];
-        qq = warp_sum(qq);
-        if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = qq;
+        __shared__ float part[NS][8];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float v = warp_sum(qq[s]);
+            if ((threadIdx.x & 31) == 0) part[s][threadIdx.x >> 5] = v;
+        }
         __syncthreads();
-        if (threadIdx.x < 32) {
-            float v = threadIdx.x < 8 ? part[threadIdx.x] : 0.f;
+        if (threadIdx.x < 32 * NS) {
+            const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
+            float v = l < 8 ? part[s][l] : 0.f;
             v = warp_sum(v);
-            if (threadIdx.x == 0) atomicAdd(red + prob, (double)v);
+            if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
         }
     }
 }
@@ -294,20 +318,26 @@ project_strip_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *_
 // (column), so the block costs 2 evaluations per candidate instead of 4, and the same expressions
 // as the forward projector decide membership and give the lengths (exact transpose).
 // red (optional) += ||out||^2 of this problem.
-template <bool POLY>
+// NS slices of the batch share one thread (same geometry, see project_kernel): the candidate's six ray_cum
+// values are computed once, each slice adds one sinogram load, one multiply and four FMAs.
+// grid.z = groups*N, group g = slices slice0 + g*NS .. + NS-1.
+template <bool POLY, int NS>
 __global__ void __launch_bounds__(128)
 backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__restrict__ views,
                    const int4 *__restrict__ split, const float *__restrict__ sino, float *__restrict__ out,
-                   double *__restrict__ red)
+                   double *__restrict__ red, int slice0)
 {
-    const int prob = blockIdx.z;
-    const int phase = prob % G.n_phase;
+    const int phase = blockIdx.z % G.n_phase;
+    const int prob = (slice0 + (blockIdx.z / G.n_phase) * NS) * G.n_phase + phase;   // of the group's first slice
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int c0 = blockIdx.x * 16 + 2 * (lane & 7);
     const int r0 = blockIdx.y * 32 + warp * 8 + 2 * (lane >> 3);
     const int V = G.n_views, B = G.n_bins;
+    const size_t img_stride = (size_t)G.n_phase * G.nx * G.ny, sino_stride = (size_t)G.n_phase * V * B;   // per slice
     const bool inside = (c0 < G.nx) && (r0 < G.ny);
-    float a00 = 0.f, a01 = 0.f, a10 = 0.f, a11 = 0.f;
+    float a00[NS], a01[NS], a10[NS], a11[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) { a00[s] = 0.f; a01[s] = 0.f; a10[s] = 0.f; a11[s] = 0.f; }
     if (inside) {
         // block centre
         const float X = ((float)c0 + 0.5f - 0.5f * (float)(G.nx - 1)) * G.pix;
@@ -328,19 +358,23 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             const float m0 = (STEEP ? cf : rf) - 1.0f, m1 = m0 + 1.0f, m2 = m0 + 2.0f;
             const float4 *__restrict__ tp = tb0 + kb0;
             const float *__restrict__ sp = sg0 + kb0;
-#pragma unroll BP_UNROLL
+#pragma unroll (NS == 1 ? BP_UNROLL : 1)
             for (int n = kb1 - kb0; n >= 0; --n, ++tp, ++sp) {
                 const float4 e4 = __ldg(tp);                 // plo, m, len (sign = steep), inva
-                const float asv = __fmul_rn(fabsf(e4.z), __ldg(sp));
+                const float alen = fabsf(e4.z);
                 const float lo0 = ray_lo(e4.x, e4.y, q0), lo1 = ray_lo(e4.x, e4.y, q1);
                 const float G00 = ray_cum(m0, lo0, e4.w), G01 = ray_cum(m1, lo0, e4.w), G02 = ray_cum(m2, lo0, e4.w);
                 const float G10 = ray_cum(m0, lo1, e4.w), G11 = ray_cum(m1, lo1, e4.w), G12 = ray_cum(m2, lo1, e4.w);
                 const float dA0 = __fsub_rn(G01, G00), dB0 = __fsub_rn(G02, G01);
                 const float dA1 = __fsub_rn(G11, G10), dB1 = __fsub_rn(G12, G11);
-                a00 = __fmaf_rn(asv, dA0, a00);
-                a11 = __fmaf_rn(asv, dB1, a11);
-                a01 = __fmaf_rn(asv, STEEP ? dB0 : dA1, a01);
-                a10 = __fmaf_rn(asv, STEEP ? dA1 : dB0, a10);
+#pragma unroll
+                for (int s = 0; s < NS; ++s) {
+                    const float asv = __fmul_rn(alen, __ldg(sp + s * sino_stride));
+                    a00[s] = __fmaf_rn(asv, dA0, a00[s]);
+                    a11[s] = __fmaf_rn(asv, dB1, a11[s]);
+                    a01[s] = __fmaf_rn(asv, STEEP ? dB0 : dA1, a01[s]);
+                    a10[s] = __fmaf_rn(asv, STEEP ? dA1 : dB0, a10[s]);
+                }
             }
         };
         int vB = 0;                                          // v * B
@@ -374,26 +408,36 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
                 run(std::false_type{}, vB + c0k, vB + k_hi);
             }
         }
-        float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + (size_t)r0 * G.nx + c0;
         const bool c1in = c0 + 1 < G.nx, r1in = r0 + 1 < G.ny;
-        if (c1in && ((G.nx & 1) == 0) && ((reinterpret_cast<uintptr_t>(out) & 7) == 0)) {
-            *reinterpret_cast<float2 *>(o) = make_float2(a00, a01);
-            if (r1in) *reinterpret_cast<float2 *>(o + G.nx) = make_float2(a10, a11);
-        } else {
-            o[0] = a00;
-            if (c1in) o[1] = a01;
-            if (r1in) { o[G.nx] = a10; if (c1in) o[G.nx + 1] = a11; }
+        const bool vec = c1in && ((G.nx & 1) == 0) && ((reinterpret_cast<uintptr_t>(out) & 7) == 0);
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + s * img_stride + (size_t)r0 * G.nx + c0;
+            if (vec) {
+                *reinterpret_cast<float2 *>(o) = make_float2(a00[s], a01[s]);
+                if (r1in) *reinterpret_cast<float2 *>(o + G.nx) = make_float2(a10[s], a11[s]);
+            } else {
+                o[0] = a00[s];
+                if (c1in) o[1] = a01[s];
+                if (r1in) { o[G.nx] = a10[s]; if (c1in) o[G.nx + 1] = a11[s]; }
+            }
+            if (!c1in) { a01[s] = 0.f; a11[s] = 0.f; }
+            if (!r1in) { a10[s] = 0.f; a11[s] = 0.f; }
         }
-        if (!c1in) { a01 = 0.f; a11 = 0.f; }
-        if (!r1in) { a10 = 0.f; a11 = 0.f; }
     }
     if (red) {
-        __shared__ float part[4];
-        float v = a00 * a00 + a01 * a01 + a10 * a10 + a11 * a11;
-        v = warp_sum(v);
-        if (lane == 0) part[warp] = v;
+        __shared__ float part[NS][4];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            float v = a00[s] * a00[s] + a01[s] * a01[s] + a10[s] * a10[s] + a11[s] * a11[s];
+            v = warp_sum(v);
+            if (lane == 0) part[s][warp] = v;
+        }
         __syncthreads();
-        if (threadIdx.x == 0) atomicAdd(red + prob, (double)(part[0] + part[1] + part[2] + part[3]));
+        if (threadIdx.x < NS) {
+            const int s = threadIdx.x;
+            atomicAdd(red + prob + s * G.n_phase, (double)(part[s][0] + part[s][1] + part[s][2] + part[s][3]));
+        }
     }
 }
 

@@ -82,6 +82,9 @@ struct SweepParams {
     int clip;               // apply max(.,0) to the output
     int ap_ns;              // gj_apply_kernel: stages of its bulk-copy ring
     int n_img;              // gj_apply2_kernel: S*N images in this launch
+    int ap_reverse;         // gj_apply2_kernel: deal the tasks from the last one down (snake order over the sweeps)
+    long long res_tasks;    // stored-weight tasks (row pairs, in layout order) below this index are kept in L2
+                            // (evict_last) by the storing sweep and the applying sweeps; the rest streams (evict_first)
 };
 
 // Shared-memory tile geometry (words), shared by host (sizing) and device.
@@ -291,8 +294,11 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     // stored-weight chunk of this warp: [W*W][RB][128] halves
     constexpr size_t WSTRIDE = (size_t)RB * SW_TW;         // halves per offset
     __nv_bfloat16 *__restrict__ wchunk = nullptr;
+    uint64_t wpol = 0;                                     // L2 policy of this chunk's stores (see SweepParams::res_tasks)
     if (STORE_W) {
         const size_t gband = (size_t)(tile_r0 / RB) + band, tx = tile_c0 / SW_TW;
+        const long long chunk = ((long long)img * ((ny + RB - 1) / RB) + (long long)gband) * p.tiles_x + (long long)tx;
+        wpol = (r0 < ny && chunk * (RB / 2) < p.res_tasks) ? l2_policy_evict_last() : l2_policy_evict_first();
         wchunk = wts + ((((size_t)img * 2 + side) * p.nbands + gband) * p.tiles_x + tx) *
                            (size_t)((2 * a + 1) * (2 * a + 1)) * WSTRIDE;
     }
@@ -393,7 +399,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
                         // 16-byte stride cost 20 us more per cfg-2 sweep)
                         if (rr & 1) {
                             if (dc0 + gg <= a)     // (rows / columns past the image edge land in chunk padding)
-                                *reinterpret_cast<uint4 *>(witem + gg * WSTRIDE + (rr >> 1) * 256) = make_uint4(held[gg].x, held[gg].y, pk.x, pk.y);
+                                stg128_hint(witem + gg * WSTRIDE + (rr >> 1) * 256, make_uint4(held[gg].x, held[gg].y, pk.x, pk.y), wpol);
                         } else {
                             held[gg] = pk;
                         }
@@ -675,7 +681,10 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     const long long n_tasks = (long long)p.n_img * tiles_per_img * npairs;
     const long long n_warps = (long long)gridDim.x * wpc;
 #pragma unroll 1
-    for (long long task = (long long)blockIdx.x * wpc + warp; task < n_tasks; task += n_warps) {
+    const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
+    for (long long tk = (long long)blockIdx.x * wpc + warp; tk < n_tasks; tk += n_warps) {
+        const long long task = p.ap_reverse ? n_tasks - 1 - tk : tk;
+        const uint64_t pol = task < p.res_tasks ? pol_keep : pol_stream;
         const int pair = (int)(task % npairs);
         const long long chunk = task / npairs;               // (img, gband, tx)
         const int img = (int)(chunk / tiles_per_img);
@@ -697,10 +706,14 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
             cp_async_commit();
             const uint4 *__restrict__ nextp = ws;             // piece `issued` of this side
             unsigned issued = 0;
+            // (the write slot is a per-lane running address: with a uniform ring offset ptxas folds it into
+            // [R + UR] addressing, and an LDGSTS that also carries an L2 policy in desc[UR] then faults)
+            unsigned wr = ring_s;
 #pragma unroll 1
             for (; issued < DEPTH - 1; ++issued, nextp += pstride) {
-                cp_async16_s(ring_s + ((issued & (DEPTH - 1)) << 9), nextp, issued < (unsigned)WW);
+                cp_async16_s_hint(wr, nextp, issued < (unsigned)WW, pol);
                 cp_async_commit();
+                wr += 512;
             }
             cp_async_wait<DEPTH - 1>();                       // the window has landed (every lane's part of it)
             __syncwarp();
@@ -719,9 +732,10 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
 #pragma unroll
                     for (int jj = 0; jj < 4; ++jj) {
                         if (jj < noff) {
-                            cp_async16_s(ring_s + ((issued & (DEPTH - 1)) << 9), nextp, issued < (unsigned)WW);
+                            cp_async16_s_hint(wr, nextp, issued < (unsigned)WW, pol);
                             cp_async_commit();                // (empty groups keep the wait count uniform)
                             ++issued; nextp += pstride;
+                            wr = (wr == ring_s + (DEPTH - 1) * 512) ? ring_s : wr + 512;
                             cp_async_wait<DEPTH - 1>();       // piece t has landed (this lane's own 16 bytes)
                             const uint4 wv = lds128_s(ring_s + ((t & (DEPTH - 1)) << 9));
                             ++t;

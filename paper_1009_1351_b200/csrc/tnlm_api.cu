@@ -49,6 +49,10 @@ struct tnlm_handle {
     int opt_apply = 1;      // 1: gj_apply2_kernel (persistent warp tasks, cp.async rings); 0: gj_apply_kernel (TMA ring)
     int opt_depth = 0;      // gj_apply2_kernel ring depth override (0 = cost model)
     int opt_wpc = 0;        // gj_apply2_kernel warps per CTA override (0 = cost model)
+    int opt_project_group = 1;      // project_kernel: at most this many slices of a batch per thread (4, 2 or 1)
+    int opt_backproject_group = 8;  // backproject_kernel: the same (8, 4, 2 or 1)
+    int opt_snake = 1;      // gj_apply2_kernel: successive sweeps deal their tasks in opposite orders
+    long long opt_resident_mb = 32;   // MB of stored weights marked evict_last in L2 (the rest evict_first); 0 = none
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
     RayRange *d_rng = nullptr;
@@ -534,21 +538,49 @@ static int launch_project(tnlm_handle *H, const float *img, const float *imgT, c
         const int tasks = H->G.n_views * ((H->G.n_bins + 31) / 32);
         dim3 grid((tasks + PS_WARPS - 1) / PS_WARPS, n_slices * H->n_phase);
         project_strip_kernel<MODE><<<grid, 32 * PS_WARPS, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red);
-    } else {
-        dim3 grid((nray + 255) / 256, n_slices * H->n_phase);
-        project_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red);
+        LAUNCHED(H);
+        return TNLM_OK;
     }
-    LAUNCHED(H);
+    // slices of a batch share the geometry: groups of 4 (then 2, then 1) slices per thread (project_kernel)
+    const int max_ns = H->opt_project_group;
+    int s0 = 0;
+    for (int ns = 4; ns >= 1; ns >>= 1) {
+        if (ns > max_ns) continue;
+        const int groups = (n_slices - s0) / ns;
+        if (groups < 1) continue;
+        dim3 grid((nray + 255) / 256, groups * H->n_phase);
+        if (ns == 4) project_kernel<MODE, 4><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
+        else if (ns == 2) project_kernel<MODE, 2><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
+        else project_kernel<MODE, 1><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
+        LAUNCHED(H);
+        s0 += groups * ns;
+    }
+    return TNLM_OK;
+}
+template <bool POLY>
+static int launch_backproject_groups(tnlm_handle *H, const float *sino, float *img, double *red, int n_slices, cudaStream_t st)
+{
+    const int max_ns = H->opt_backproject_group;
+    int s0 = 0;
+    for (int ns = 8; ns >= 1; ns >>= 1) {
+        if (ns > max_ns) continue;
+        const int groups = (n_slices - s0) / ns;
+        if (groups < 1) continue;
+        dim3 grid((H->nx + 15) / 16, (H->ny + 31) / 32, groups * H->n_phase);
+        if (ns == 8) backproject_kernel<POLY, 8><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        else if (ns == 4) backproject_kernel<POLY, 4><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        else if (ns == 2) backproject_kernel<POLY, 2><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        else backproject_kernel<POLY, 1><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        LAUNCHED(H);
+        s0 += groups * ns;
+    }
     return TNLM_OK;
 }
 static int launch_backproject(tnlm_handle *H, const float *sino, float *img, double *red, int n_slices, cudaStream_t st)
 {
     ProfScope ps(H, TNLM_KERNEL_BACKPROJECT, st);
-    dim3 grid((H->nx + 15) / 16, (H->ny + 31) / 32, n_slices * H->n_phase);
-    if (H->fan_poly) backproject_kernel<true><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red);
-    else backproject_kernel<false><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red);
-    LAUNCHED(H);
-    return TNLM_OK;
+    return H->fan_poly ? launch_backproject_groups<true>(H, sino, img, red, n_slices, st)
+                       : launch_backproject_groups<false>(H, sino, img, red, n_slices, st);
 }
 
 extern "C" int tnlm_project(tnlm_handle *H, const float *img, float *sino, int n_slices, void *stream)
@@ -710,6 +742,14 @@ static void fill_layout(const tnlm_handle *H, const SweepShape &sh, SweepParams 
     R.nbands = R.tiles_y * sh.nb;
 }
 
+// Stored-weight tasks (row pairs of 2 x 128 pixels, both sides: 2 W^2 pieces of 512 bytes) the option
+// apply_resident_mb keeps in L2.
+static long long resident_tasks(const tnlm_handle *H)
+{
+    const double task_bytes = 2.0 * H->window * H->window * 512.0;
+    return (long long)((double)H->opt_resident_mb * 1048576.0 / task_bytes);
+}
+
 // One sweep with the weights computed on the fly; wts != NULL also stores them (bf16 chunks).
 static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
                         int n_slices, __nv_bfloat16 *wts, cudaStream_t st)
@@ -718,6 +758,7 @@ static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, co
     SweepParams R = H->R;
     R.clip = clip;
     fill_layout(H, sh, R);
+    R.res_tasks = resident_tasks(H);
     const long long ctas = (long long)nimg * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
     void *args[] = {(void *)&R, (void *)&g, (void *)&u, (void *)&out, (void *)&wts};
@@ -730,10 +771,14 @@ static int launch_sweep(tnlm_handle *H, const SweepShape &sh, const float *g, co
 
 // One sweep with the stored weights of this outer iteration (written by shape sh).
 static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, const float *u, float *out, int clip,
-                        int n_slices, const __nv_bfloat16 *wts, cudaStream_t st)
+                        int n_slices, const __nv_bfloat16 *wts, int sweep_index, cudaStream_t st)
 {
     SweepParams R = H->R;
     R.clip = clip;
+    R.res_tasks = resident_tasks(H);
+    // the storing sweep (index 0) wrote the chunks front to back: sweep 1 starts from the back, where the
+    // freshest lines are, sweep 2 from the front, ...
+    R.ap_reverse = (H->opt_snake && (sweep_index & 1)) ? 1 : 0;
     fill_layout(H, sh, R);
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
@@ -892,6 +937,10 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
     else if (n == "apply_depth") { if ((ok = (value == 0 || value == 4 || value == 8 || value == 16))) H->opt_depth = (int)value; }
     else if (n == "apply_wpc") { if ((ok = (value == 0 || in(2, 8)))) H->opt_wpc = (int)value; }
+    else if (n == "project_group") { if ((ok = (value == 1 || value == 2 || value == 4))) H->opt_project_group = (int)value; }
+    else if (n == "backproject_group") { if ((ok = (value == 1 || value == 2 || value == 4 || value == 8))) H->opt_backproject_group = (int)value; }
+    else if (n == "apply_snake") { if ((ok = in(0, 1))) H->opt_snake = (int)value; }
+    else if (n == "apply_resident_mb") { if ((ok = in(0, 1 << 20))) H->opt_resident_mb = value; }
     else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);
     if (!ok) return fail(H, TNLM_INVALID_ARG, "value out of range for option " + n);
     return TNLM_OK;
@@ -933,7 +982,7 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
         else { dst = pp[which]; if (dst == src) { which ^= 1; dst = pp[which]; } }
         const bool computes = (m == 0 || !wts);
         if (computes) rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
-        else rc = launch_apply(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, st);
+        else rc = launch_apply(H, *sh, g, src, dst, last ? 1 : 0, n_slices, wts, m, st);
         if (rc) return rc;
         src = dst;
         which ^= 1;

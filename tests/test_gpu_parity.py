@@ -182,6 +182,35 @@ def test_strip_and_gather_forward_projectors_are_bit_identical(T, cfg):
     assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
 
 
+def test_slice_groups_share_geometry_bit_identically(T):
+    # Slices of a batch have one geometry: the projectors serve groups of 8/4/2/1 slices per thread
+    # (options backproject_group, project_group).  S = 11 = 8 + 2 + 1 exercises every group size and the
+    # remainders; per slice the arithmetic is that of a single slice: bit-identical, and equal to the oracle.
+    torch, tn = T
+    cfg = small_geom_cfg(L=37, N=2, V=23, B=61)
+    hd, og = handles(tn, cfg)
+    S = 11
+    rng = np.random.default_rng(5)
+    img = rng.random((S, cfg.N, cfg.L, cfg.L)) * 0.02
+    sino = rng.random((S, cfg.N, cfg.V, cfg.B))
+    w = rng.random((S, cfg.N, cfg.V, cfg.B)) * 50 + 1
+    imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
+    ref = {}
+    for pg, bg in [(1, 1), (2, 2), (4, 4), (4, 8), (1, 8)]:
+        tn.set_option(hd, "project_kernel", 0); tn.set_option(hd, "project_group", pg); tn.set_option(hd, "backproject_group", bg)
+        po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
+        tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo)
+        tn.cgls_step(hd, imgd, sinod, wd, 2, go)          # fused epilogues and per-problem reductions of every slice
+        if not ref:
+            ref = dict(p=po, b=bo, g=go)
+            for s in (0, 7, 8, 10):
+                assert rel(po[s].cpu().numpy(), oracle.project(og, img[s])) < 2e-6
+                assert rel(bo[s].cpu().numpy(), oracle.backproject(og, sino[s], cfg.L, cfg.L)) < 2e-6
+                assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 2)) < STEP_TOL
+        else:
+            assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg)
+
+
 @pytest.mark.parametrize("B,V", [(120, 16), (200, 9)], ids=["fan76", "fan127"])
 def test_backprojector_candidate_range_misses_no_ray(T, B, V):
     # The gather's candidate bins per (2 x 2 block, view) are a conservative range around the block centre's fan
@@ -343,6 +372,13 @@ def test_both_stored_weight_sweep_kernels_agree(T):
             out = torch.empty_like(gd)
             tn.regularize_step(hd, gd, m2, out)
             assert torch.equal(out, ref), (W, depth, wpc)
+        # task order (snake over the sweeps) and L2 residency hints change where bytes come from, not one bit
+        tn.set_option(hd, "apply_depth", 0); tn.set_option(hd, "apply_wpc", 0)
+        for snake, mb in [(0, 0), (1, 0), (0, 1), (1, 1), (1, 4096)]:
+            tn.set_option(hd, "apply_snake", snake); tn.set_option(hd, "apply_resident_mb", mb)
+            out = torch.empty_like(gd)
+            tn.regularize_step(hd, gd, m2, out)
+            assert torch.equal(out, ref), (W, snake, mb)
 
 
 def test_regularize_multi_slice_equals_per_slice(T):
