@@ -310,18 +310,18 @@ project_strip_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *_
 }
 
 // ----------------------------------------------------------------------------- adjoint
-// grid = (ceil(nx/16), ceil(ny/32), S*N); block = 128 threads.  One thread per 2 x 2 pixel block
-// (rows r0, r0+1, columns c0, c0+1; a warp covers 16 x 8 pixels), loop over the views of its
-// phase.  Per view the candidate bins are those whose fan angle is within the block's angular
-// footprint (conservative superset).  A steep candidate is evaluated in rows r0 and r0+1, a
-// shallow one in columns c0 and c0+1: each evaluation serves the two block pixels of that row
-// (column), so the block costs 2 evaluations per candidate instead of 4, and the same expressions
-// as the forward projector decide membership and give the lengths (exact transpose).
-// red (optional) += ||out||^2 of this problem.
-// NS slices of the batch share one thread (same geometry, see project_kernel): the candidate's six ray_cum
-// values are computed once, each slice adds one sinogram load, one multiply and four FMAs.
-// grid.z = groups*N, group g = slices slice0 + g*NS .. + NS-1.
-template <bool POLY, int NS>
+// One thread per BR x BC pixel block (rows r0 .. r0+BR-1, columns c0 .. c0+BC-1; a warp covers 4 x 8 blocks, a CTA
+// of 4 warps 16 x 8 blocks), loop over the views of its phase.  Per view the candidate bins are those whose fan angle
+// is within the block's angular footprint (conservative superset).  A steep candidate is evaluated in the block's
+// BR rows, a shallow one in its BC columns: one evaluation of a line serves all block pixels of that line with the
+// cumulative fraction F (ray_cum) at their cell boundaries, so the same expressions as the forward projector decide
+// membership and give the lengths (exact transpose), and the per-view work (fan angle, candidate range, the runs of
+// ray classes) is shared by BR*BC pixels.
+// NS slices of the batch share one thread (same geometry, see project_kernel): the candidate's ray_cum values are
+// computed once, each slice adds one sinogram load, one multiply and BR*BC FMAs.
+// grid = (ceil(nx/(8 BC)), ceil(ny/(16 BR)), groups*N), group g = slices slice0 + g*NS .. + NS-1; block = 128.
+// red (optional) += ||out||^2 of every problem.
+template <bool POLY, int NS, int BR, int BC>
 __global__ void __launch_bounds__(128)
 backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__restrict__ views,
                    const int4 *__restrict__ split, const float *__restrict__ sino, float *__restrict__ out,
@@ -330,50 +330,62 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
     const int phase = blockIdx.z % G.n_phase;
     const int prob = (slice0 + (blockIdx.z / G.n_phase) * NS) * G.n_phase + phase;   // of the group's first slice
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int c0 = blockIdx.x * 16 + 2 * (lane & 7);
-    const int r0 = blockIdx.y * 32 + warp * 8 + 2 * (lane >> 3);
+    const int c0 = (blockIdx.x * 8 + (lane & 7)) * BC;
+    const int r0 = (blockIdx.y * 16 + warp * 4 + (lane >> 3)) * BR;
     const int V = G.n_views, B = G.n_bins;
     const size_t img_stride = (size_t)G.n_phase * G.nx * G.ny, sino_stride = (size_t)G.n_phase * V * B;   // per slice
     const bool inside = (c0 < G.nx) && (r0 < G.ny);
-    float a00[NS], a01[NS], a10[NS], a11[NS];
+    float acc[NS][BR][BC];
 #pragma unroll
-    for (int s = 0; s < NS; ++s) { a00[s] = 0.f; a01[s] = 0.f; a10[s] = 0.f; a11[s] = 0.f; }
+    for (int s = 0; s < NS; ++s)
+#pragma unroll
+        for (int j = 0; j < BR; ++j)
+#pragma unroll
+            for (int k = 0; k < BC; ++k) acc[s][j][k] = 0.f;
     if (inside) {
         // block centre
-        const float X = ((float)c0 + 0.5f - 0.5f * (float)(G.nx - 1)) * G.pix;
-        const float Y = ((float)r0 + 0.5f - 0.5f * (float)(G.ny - 1)) * G.pix;
+        const float X = ((float)c0 + 0.5f * (float)(BC - 1) - 0.5f * (float)(G.nx - 1)) * G.pix;
+        const float Y = ((float)r0 + 0.5f * (float)(BR - 1) - 0.5f * (float)(G.ny - 1)) * G.pix;
         const float rf = (float)r0, cf = (float)c0;
         const float4 *__restrict__ vt = views + (size_t)phase * V;
         const int4 *__restrict__ spl = split + (size_t)phase * V;
         const float4 *__restrict__ tb0 = reinterpret_cast<const float4 *>(tab + (size_t)phase * V * B);
         const float *__restrict__ sg0 = sino + (size_t)prob * V * B;
         // Candidates kb0..kb1 (offsets into the phase's table / the sinogram) of ONE class: steep rays are evaluated
-        // in rows r0, r0+1 and the block's two pixels of a row sit at minor-axis indices c0, c0+1; shallow rays in
-        // columns c0, c0+1 with minor-axis indices r0, r0+1.  The two pixels of line j get alen * (F(cA+1) - F(cA))
-        // and alen * (F(cA+2) - F(cA+1)), F = ray_cum (common.cuh): zero for cells the ray misses, and bit for bit
-        // the forward projector's entry for the cells it touches -- no membership test anywhere.
+        // in the block's rows, where its pixels sit at minor-axis indices c0 .. c0+BC-1; shallow rays in its columns
+        // with minor-axis indices r0 .. r0+BR-1.  Pixel n of a line gets alen * (F(cA+n+1) - F(cA+n)), F = ray_cum
+        // (common.cuh): zero for cells the ray misses, and bit for bit the forward projector's entry for the cells
+        // it touches -- no membership test anywhere.
         auto run = [&](auto steep_c, int kb0, int kb1) {
             constexpr bool STEEP = decltype(steep_c)::value;
-            const float q0 = STEEP ? rf : cf, q1 = q0 + 1.0f;
-            const float m0 = (STEEP ? cf : rf) - 1.0f, m1 = m0 + 1.0f, m2 = m0 + 2.0f;
+            constexpr int NL = STEEP ? BR : BC, NP = STEEP ? BC : BR;      // lines, pixels per line
+            const float q0 = STEEP ? rf : cf, m0 = (STEEP ? cf : rf) - 1.0f;
             const float4 *__restrict__ tp = tb0 + kb0;
             const float *__restrict__ sp = sg0 + kb0;
-#pragma unroll (NS == 1 ? BP_UNROLL : 1)
+#pragma unroll (NS == 1 && BR * BC == 4 ? BP_UNROLL : 1)
             for (int n = kb1 - kb0; n >= 0; --n, ++tp, ++sp) {
                 const float4 e4 = __ldg(tp);                 // plo, m, len (sign = steep), inva
                 const float alen = fabsf(e4.z);
-                const float lo0 = ray_lo(e4.x, e4.y, q0), lo1 = ray_lo(e4.x, e4.y, q1);
-                const float G00 = ray_cum(m0, lo0, e4.w), G01 = ray_cum(m1, lo0, e4.w), G02 = ray_cum(m2, lo0, e4.w);
-                const float G10 = ray_cum(m0, lo1, e4.w), G11 = ray_cum(m1, lo1, e4.w), G12 = ray_cum(m2, lo1, e4.w);
-                const float dA0 = __fsub_rn(G01, G00), dB0 = __fsub_rn(G02, G01);
-                const float dA1 = __fsub_rn(G11, G10), dB1 = __fsub_rn(G12, G11);
+                float d[NL][NP];
+#pragma unroll
+                for (int l = 0; l < NL; ++l) {
+                    const float lo = ray_lo(e4.x, e4.y, q0 + (float)l);
+                    float Gp = ray_cum(m0, lo, e4.w);
+#pragma unroll
+                    for (int n2 = 0; n2 < NP; ++n2) {
+                        const float Gn = ray_cum(m0 + (float)(n2 + 1), lo, e4.w);
+                        d[l][n2] = __fsub_rn(Gn, Gp);
+                        Gp = Gn;
+                    }
+                }
 #pragma unroll
                 for (int s = 0; s < NS; ++s) {
                     const float asv = __fmul_rn(alen, __ldg(sp + s * sino_stride));
-                    a00[s] = __fmaf_rn(asv, dA0, a00[s]);
-                    a11[s] = __fmaf_rn(asv, dB1, a11[s]);
-                    a01[s] = __fmaf_rn(asv, STEEP ? dB0 : dA1, a01[s]);
-                    a10[s] = __fmaf_rn(asv, STEEP ? dA1 : dB0, a10[s]);
+#pragma unroll
+                    for (int j = 0; j < BR; ++j)
+#pragma unroll
+                        for (int k = 0; k < BC; ++k)
+                            acc[s][j][k] = __fmaf_rn(asv, STEEP ? d[j][k] : d[k][j], acc[s][j][k]);
                 }
             }
         };
@@ -388,10 +400,11 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rdot) : "f"(dot));
             const float t = crs * rdot;
             const float kc = fmaf(POLY ? fan_angle_poly(t) : atanf(t), G.sdd_over_pitch, G.bin_centre);
-            // a ray crosses the 2 x 2 block (half-side pix) iff it passes within pix*(|nx|+|ny|) of its centre, n the
-            // ray's unit normal ~ (-py, px)/d: angular half-width pix*(|px|+|py|)/d^2 <= pix*(|px|+|py|)/dot^2
-            // (hw_scale carries pix, bins per radian and 2 % for the second-order terms), + 0.05 bin of rounding
-            const float hw = fmaf(G.hw_scale * (fabsf(px) + fabsf(py)), rdot * rdot, 0.05f);
+            // a ray crosses the block (half-sides hx = BC/2, hy = BR/2 pixels) iff it passes within
+            // pix*(hx*|nx| + hy*|ny|) of its centre, n the ray's unit normal ~ (-py, px)/d: angular half-width
+            // pix*(hx*|py| + hy*|px|)/d^2 <= .../dot^2 (hw_scale carries pix, bins per radian and 2 % for the
+            // second-order terms), + 0.05 bin of rounding
+            const float hw = fmaf(G.hw_scale * (0.5f * (float)BC * fabsf(py) + 0.5f * (float)BR * fabsf(px)), rdot * rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             // the steep / shallow classes are contiguous runs of the bin index (a fan narrower than 90 degrees crosses a
@@ -408,28 +421,36 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
                 run(std::false_type{}, vB + c0k, vB + k_hi);
             }
         }
-        const bool c1in = c0 + 1 < G.nx, r1in = r0 + 1 < G.ny;
-        const bool vec = c1in && ((G.nx & 1) == 0) && ((reinterpret_cast<uintptr_t>(out) & 7) == 0);
+        const bool full = (c0 + BC <= G.nx);
+        const bool vec = full && ((G.nx & (BC - 1)) == 0) && ((reinterpret_cast<uintptr_t>(out) & (4 * BC - 1)) == 0);
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
             float *__restrict__ o = out + (size_t)prob * G.nx * G.ny + s * img_stride + (size_t)r0 * G.nx + c0;
-            if (vec) {
-                *reinterpret_cast<float2 *>(o) = make_float2(a00[s], a01[s]);
-                if (r1in) *reinterpret_cast<float2 *>(o + G.nx) = make_float2(a10[s], a11[s]);
-            } else {
-                o[0] = a00[s];
-                if (c1in) o[1] = a01[s];
-                if (r1in) { o[G.nx] = a10[s]; if (c1in) o[G.nx + 1] = a11[s]; }
+#pragma unroll
+            for (int j = 0; j < BR; ++j) {
+                const bool rin = r0 + j < G.ny;
+                if (rin && vec) {
+                    if (BC == 4) *reinterpret_cast<float4 *>(o + (size_t)j * G.nx) = make_float4(acc[s][j][0], acc[s][j][1], acc[s][j][BC > 2 ? 2 : 0], acc[s][j][BC > 3 ? 3 : 0]);
+                    else *reinterpret_cast<float2 *>(o + (size_t)j * G.nx) = make_float2(acc[s][j][0], acc[s][j][1]);
+                }
+#pragma unroll
+                for (int k = 0; k < BC; ++k) {
+                    const bool in = rin && (c0 + k < G.nx);
+                    if (in && !vec) o[(size_t)j * G.nx + k] = acc[s][j][k];
+                    if (!in) acc[s][j][k] = 0.f;             // (not part of the image: keep it out of the norm)
+                }
             }
-            if (!c1in) { a01[s] = 0.f; a11[s] = 0.f; }
-            if (!r1in) { a10[s] = 0.f; a11[s] = 0.f; }
         }
     }
     if (red) {
         __shared__ float part[NS][4];
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
-            float v = a00[s] * a00[s] + a01[s] * a01[s] + a10[s] * a10[s] + a11[s] * a11[s];
+            float v = 0.f;
+#pragma unroll
+            for (int j = 0; j < BR; ++j)
+#pragma unroll
+                for (int k = 0; k < BC; ++k) v = fmaf(acc[s][j][k], acc[s][j][k], v);
             v = warp_sum(v);
             if (lane == 0) part[s][warp] = v;
         }

@@ -659,6 +659,8 @@ __host__ __device__ inline size_t apply2_warp_bytes(int window, int depth)
     return (size_t)(2 + 2 * a) * apply_uw(window) * sizeof(float) + (size_t)depth * 512;
 }
 
+// Tried and dropped: writing the weight sums Z in the first applying sweep and reading them back in the later ones
+// (8 fewer instructions per 512-byte piece) leaves the sweep at the same 61.8 us: it waits for bytes, not for issue slots.
 template <int DEPTH>             // pieces in flight per warp (a power of two)
 __global__ void __launch_bounds__(256, 2)
 gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
@@ -680,11 +682,14 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
     const long long n_tasks = (long long)p.n_img * tiles_per_img * npairs;
     const long long n_warps = (long long)gridDim.x * wpc;
-#pragma unroll 1
     const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
-    for (long long tk = (long long)blockIdx.x * wpc + warp; tk < n_tasks; tk += n_warps) {
+#pragma unroll 1
+    for (long long base = (long long)blockIdx.x * wpc; base < n_tasks; base += n_warps) {
+        // (the L2 policy is chosen per CTA and round, from `base`: uniform, so it lives in a uniform register)
+        const uint64_t pol = (p.ap_reverse ? n_tasks - 1 - base : base) < p.res_tasks ? pol_keep : pol_stream;
+        const long long tk = base + warp;
+        if (tk >= n_tasks) break;
         const long long task = p.ap_reverse ? n_tasks - 1 - tk : tk;
-        const uint64_t pol = task < p.res_tasks ? pol_keep : pol_stream;
         const int pair = (int)(task % npairs);
         const long long chunk = task / npairs;               // (img, gband, tx)
         const int img = (int)(chunk / tiles_per_img);
@@ -715,9 +720,9 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
                 cp_async_commit();
                 wr += 512;
             }
+            float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
             cp_async_wait<DEPTH - 1>();                       // the window has landed (every lane's part of it)
             __syncwarp();
-            float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
             unsigned t = 0;
 #pragma unroll 1
             for (int dr = 0; dr < W; ++dr) {
