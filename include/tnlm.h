@@ -64,7 +64,10 @@
  *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first),
  *   backproject_group (8, the default; 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
  *   share the geometry (nothing couples them, L77), so one thread of a projector serves up to that many slices
- *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change.
+ *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change;
+ *   project_interleave (1, the default: in a call with four or more slices the forward projector reads handle-owned
+ *   copies of the image in which the four slices of a group are interleaved per pixel, one 16-byte gather per cell
+ *   for four slices; 0 = every slice from its own image and transposed copy).
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
@@ -164,7 +167,7 @@ int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_ent
 
 /* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
  * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns", "apply_kernel", "apply_depth", "apply_wpc",
- * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "backproject_group"; 0 restores the
+ * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "project_interleave", "backproject_group"; 0 restores the
  * heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
 int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
 

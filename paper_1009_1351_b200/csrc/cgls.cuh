@@ -62,15 +62,15 @@ cgls_update_r(float *__restrict__ r, float *__restrict__ rw, const float *__rest
 // u += a_m s (step 2, L114) and, unless LAST, s = t + b_m s (step 5, L126) with the transposed copy sT
 // the forward projector reads for its shallow rays, in one pass over 32 x 32 image tiles.
 // A broken-down phase has a = b = 0: u stays, s = t (never used again).
-// grid = (ceil(nx/32), ceil(ny/32), nprob); block = (32, 8).
+// grid = (ceil(nx/32), ceil(ny/32), problems prob0 .. ); block = (32, 8).
 template <bool LAST>
 __global__ void __launch_bounds__(256)
 cgls_update_us(float *__restrict__ u, float *__restrict__ s, const float *__restrict__ t, float *__restrict__ sT,
-               int nx, int ny, const double *gam, const double *qq, int nprob, int m)
+               int nx, int ny, const double *gam, const double *qq, int nprob, int m, int prob0)
 {
     __shared__ float tile[32][33];
     __shared__ float ab[2];
-    const int prob = blockIdx.z;
+    const int prob = blockIdx.z + prob0;
     if (threadIdx.x == 0 && threadIdx.y == 0) {
         ab[0] = cgls_a(gam, qq, nprob, prob, m);
         ab[1] = LAST ? 0.f : cgls_b(gam, qq, nprob, prob, m);
@@ -101,6 +101,60 @@ cgls_update_us(float *__restrict__ u, float *__restrict__ s, const float *__rest
     for (int j = 0; j < 32; j += 8) {
         const int cT = blockIdx.x * 32 + threadIdx.y + j;
         if (rT < ny && cT < nx) sT[base + (size_t)cT * ny + rT] = tile[threadIdx.x][threadIdx.y + j];
+    }
+}
+
+// The same for a group of four slices whose search direction s lives only in the interleaved copies the batch
+// projector reads (project_il_kernel): sI[group][phase][r][c] = s of slices 4g .. 4g+3, updated in place, and its
+// transpose sTI; u and t stay in the caller's layout.  Per slice the arithmetic is that of cgls_update_us.
+// grid = (ceil(nx/32), ceil(ny/32), groups*N); block = (32, 8).
+template <bool LAST>
+__global__ void __launch_bounds__(256)
+cgls_update_us_il(float *__restrict__ u, float4 *__restrict__ sI, const float *__restrict__ t, float4 *__restrict__ sTI,
+                  int nx, int ny, int n_phase, const double *gam, const double *qq, int nprob, int m)
+{
+    __shared__ float4 tile[32][33];
+    __shared__ float ab[2][4];
+    const int group = blockIdx.z / n_phase, phase = blockIdx.z - group * n_phase;
+    const int prob = group * 4 * n_phase + phase;            // of the group's first slice
+    if (threadIdx.y == 0 && threadIdx.x < 4) {
+        ab[0][threadIdx.x] = cgls_a(gam, qq, nprob, prob + threadIdx.x * n_phase, m);
+        ab[1][threadIdx.x] = LAST ? 0.f : cgls_b(gam, qq, nprob, prob + threadIdx.x * n_phase, m);
+    }
+    __syncthreads();
+    const float a[4] = {ab[0][0], ab[0][1], ab[0][2], ab[0][3]}, b[4] = {ab[1][0], ab[1][1], ab[1][2], ab[1][3]};
+    const size_t npix = (size_t)nx * ny, sl = (size_t)n_phase * npix;
+    const size_t base = (size_t)prob * npix, base4 = ((size_t)group * n_phase + phase) * npix;
+    const int c = blockIdx.x * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int r = blockIdx.y * 32 + threadIdx.y + j;
+        float4 sn = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (r < ny && c < nx) {
+            const size_t o = (size_t)r * nx + c;
+            const float4 so4 = sI[base4 + o];
+            const float so[4] = {so4.x, so4.y, so4.z, so4.w};
+            float snv[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const size_t oq = base + q * sl + o;
+                u[oq] = fmaf(a[q], so[q], u[oq]);
+                if (!LAST) snv[q] = fmaf(b[q], so[q], t[oq]);
+            }
+            if (!LAST) {
+                sn = make_float4(snv[0], snv[1], snv[2], snv[3]);
+                sI[base4 + o] = sn;
+            }
+        }
+        if (!LAST) tile[threadIdx.y + j][threadIdx.x] = sn;
+    }
+    if (LAST) return;
+    __syncthreads();
+    const int rT = blockIdx.y * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int cT = blockIdx.x * 32 + threadIdx.y + j;
+        if (rT < ny && cT < nx) sTI[base4 + (size_t)cT * ny + rT] = tile[threadIdx.x][threadIdx.y + j];
     }
 }
 

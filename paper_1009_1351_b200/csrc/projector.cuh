@@ -50,10 +50,10 @@ __device__ __forceinline__ float fan_angle_poly(float t)
 // sit in ~18 different image rows there (18 cache lines per load); in the transposed copy they are
 // neighbours again.  grid = (ceil(nx/32), ceil(ny/32), S*N), block = (32, 8).
 __global__ void __launch_bounds__(256)
-transpose_kernel(const float *__restrict__ img, float *__restrict__ imgT, int nx, int ny)
+transpose_kernel(const float *__restrict__ img, float *__restrict__ imgT, int nx, int ny, int prob0)
 {
     __shared__ float tile[32][33];
-    const size_t base = (size_t)blockIdx.z * nx * ny;
+    const size_t base = (size_t)(blockIdx.z + prob0) * nx * ny;
     const int c = blockIdx.x * 32 + threadIdx.x;
 #pragma unroll
     for (int j = 0; j < 32; j += 8) {
@@ -127,6 +127,141 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
                     acc0[s] = fmaf(F1, __ldg(cell + s * img_stride), acc0[s]);
                     acc1[s] = fmaf(U1, __ldg(cell + s * img_stride + 1), acc1[s]);
                 }
+            }
+            edge(rg.ihi + 1, rg.hi);
+        } else {
+            edge(rg.lo, rg.hi);
+        }
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float p = __fmul_rn(alen, acc0[s] + acc1[s]);
+            const size_t o = (size_t)prob * nray + s * sino_stride + ray;
+            if (MODE == FWD_PLAIN) {
+                out0[o] = p;
+            } else {
+                const float sw = sw_ ? sw_[o] : 1.0f;
+                if (MODE == FWD_RESID) {
+                    const float r = sw * (y[o] - p);
+                    out0[o] = r;
+                    out1[o] = sw * r;
+                } else {
+                    const float q = sw * p;
+                    out0[o] = q;
+                    qq[s] = q * q;
+                }
+            }
+        }
+    }
+    if (MODE == FWD_SCALE) {
+        __shared__ float part[NS][8];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float v = warp_sum(qq[s]);
+            if ((threadIdx.x & 31) == 0) part[s][threadIdx.x >> 5] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x < 32 * NS) {
+            const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
+            float v = l < 8 ? part[s][l] : 0.f;
+            v = warp_sum(v);
+            if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
+        }
+    }
+}
+
+// ---- four slices interleaved per pixel -------------------------------------------------------------------------
+// project_kernel is bound by the load/store unit: two 32-lane gathers per (ray, row), ~1.8 cycles of LSU issue each
+// per SM whatever the width of the load.  For a batch the projector therefore reads copies of the image in which
+// the four slices of a group sit side by side per pixel, imI[group][phase][r][c] = (slice 4g .. 4g+3) as one float4
+// and the same transposed (imTI[group][phase][c][r]): one LDG.128 per cell serves four slices, i.e. half a gather
+// per (ray, row, slice) instead of two, and the ray walk (ray_frac) is shared as in project_kernel<., NS>.  Per
+// slice the arithmetic and its order are unchanged (bit-identical results).  The copies are made by
+// interleave4_kernel for the first P of a call and by cgls_update_us_il afterwards.
+// grid = (ceil(nx/32), ceil(ny/32), groups*N), block = (32, 8).
+__global__ void __launch_bounds__(256)
+interleave4_kernel(const float *__restrict__ img, float4 *__restrict__ imI, float4 *__restrict__ imTI, int nx, int ny,
+                   int n_phase)
+{
+    __shared__ float4 tile[32][33];
+    const int group = blockIdx.z / n_phase, phase = blockIdx.z - group * n_phase;
+    const size_t npix = (size_t)nx * ny, sl = (size_t)n_phase * npix;                 // slice stride
+    const float *__restrict__ src = img + ((size_t)group * 4 * n_phase + phase) * npix;
+    const size_t base4 = ((size_t)group * n_phase + phase) * npix;
+    const int c = blockIdx.x * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int r = blockIdx.y * 32 + threadIdx.y + j;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (r < ny && c < nx) {
+            const size_t o = (size_t)r * nx + c;
+            v = make_float4(__ldg(src + o), __ldg(src + sl + o), __ldg(src + 2 * sl + o), __ldg(src + 3 * sl + o));
+            imI[base4 + o] = v;
+        }
+        tile[threadIdx.y + j][threadIdx.x] = v;
+    }
+    __syncthreads();
+    const int rT = blockIdx.y * 32 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 32; j += 8) {
+        const int cT = blockIdx.x * 32 + threadIdx.y + j;
+        if (rT < ny && cT < nx) imTI[base4 + (size_t)cT * ny + rT] = tile[threadIdx.x][threadIdx.y + j];
+    }
+}
+
+// grid = (ceil(V*B/256), groups*N); group g = slices 4g .. 4g+3 (the groups start at slice 0).
+template <int MODE>
+__global__ void __launch_bounds__(256)
+project_il_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restrict__ rng,
+                  const float4 *__restrict__ imI, const float4 *__restrict__ imTI, const float *__restrict__ y,
+                  const float *__restrict__ sw_, float *__restrict__ out0, float *__restrict__ out1,
+                  double *__restrict__ red)
+{
+    constexpr int NS = 4;
+    const int group = blockIdx.y / G.n_phase, phase = blockIdx.y - group * G.n_phase;
+    const int prob = group * NS * G.n_phase + phase;         // slice*N + phase of the group's first slice
+    const int nray = G.n_views * G.n_bins;
+    const size_t sino_stride = (size_t)G.n_phase * nray;     // per slice
+    const int ray = blockIdx.x * blockDim.x + threadIdx.x;
+    float qq[NS] = {0.f, 0.f, 0.f, 0.f};
+    if (ray < nray) {
+        const RayEntry e = tab[(size_t)phase * nray + ray];
+        const RayRange rg = rng[(size_t)phase * nray + ray];
+        const float alen = fabsf(e.len);
+        float acc0[NS] = {0.f, 0.f, 0.f, 0.f}, acc1[NS] = {0.f, 0.f, 0.f, 0.f};
+        const bool steep = e.len > 0.f;
+        const int n_minor = steep ? G.nx : G.ny;
+        const float4 *__restrict__ base = (steep ? imI : imTI) + ((size_t)group * G.n_phase + phase) * G.nx * G.ny;
+        auto edge = [&](int q0, int q1) {                      // rows in which a touched cell may be outside
+            float qf = (float)q0;
+            const float4 *__restrict__ row = base + (size_t)q0 * n_minor;
+            for (int q = q0; q <= q1; ++q, qf += 1.0f, row += n_minor) {
+                int c0; float F1, U1;
+                ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+                if ((unsigned)c0 < (unsigned)n_minor) {
+                    const float4 v = __ldg(row + c0);
+                    acc0[0] = fmaf(F1, v.x, acc0[0]); acc0[1] = fmaf(F1, v.y, acc0[1]);
+                    acc0[2] = fmaf(F1, v.z, acc0[2]); acc0[3] = fmaf(F1, v.w, acc0[3]);
+                }
+                if ((unsigned)(c0 + 1) < (unsigned)n_minor) {
+                    const float4 v = __ldg(row + c0 + 1);
+                    acc1[0] = fmaf(U1, v.x, acc1[0]); acc1[1] = fmaf(U1, v.y, acc1[1]);
+                    acc1[2] = fmaf(U1, v.z, acc1[2]); acc1[3] = fmaf(U1, v.w, acc1[3]);
+                }
+            }
+        };
+        if (rg.ihi >= rg.ilo) {
+            edge(rg.lo, rg.ilo - 1);
+            float qf = (float)rg.ilo;
+            const float4 *__restrict__ row = base + (size_t)rg.ilo * n_minor;
+#pragma unroll 2
+            for (int q = rg.ilo; q <= rg.ihi; ++q, qf += 1.0f, row += n_minor) {
+                int c0; float F1, U1;
+                ray_frac(e.plo, e.m, e.inva, qf, c0, F1, U1);
+                const float4 v0 = __ldg(row + c0), v1 = __ldg(row + c0 + 1);
+                acc0[0] = fmaf(F1, v0.x, acc0[0]); acc0[1] = fmaf(F1, v0.y, acc0[1]);
+                acc0[2] = fmaf(F1, v0.z, acc0[2]); acc0[3] = fmaf(F1, v0.w, acc0[3]);
+                acc1[0] = fmaf(U1, v1.x, acc1[0]); acc1[1] = fmaf(U1, v1.y, acc1[1]);
+                acc1[2] = fmaf(U1, v1.z, acc1[2]); acc1[3] = fmaf(U1, v1.w, acc1[3]);
             }
             edge(rg.ihi + 1, rg.hi);
         } else {

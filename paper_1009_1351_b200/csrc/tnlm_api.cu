@@ -49,6 +49,7 @@ struct tnlm_handle {
     int opt_apply = 1;      // 1: gj_apply2_kernel (persistent warp tasks, cp.async rings); 0: gj_apply_kernel (TMA ring)
     int opt_depth = 0;      // gj_apply2_kernel ring depth override (0 = cost model)
     int opt_wpc = 0;        // gj_apply2_kernel warps per CTA override (0 = cost model)
+    int opt_project_il = 1;         // forward projector: groups of four slices read interleaved copies (project_il_kernel)
     int opt_project_group = 1;      // project_kernel: at most this many slices of a batch per thread (4, 2 or 1)
     int opt_backproject_group = 8;  // backproject_kernel: the same (8, 4, 2 or 1)
     int opt_snake = 1;      // gj_apply2_kernel: successive sweeps deal their tasks in opposite orders
@@ -67,6 +68,7 @@ struct tnlm_handle {
     float *d_s = nullptr, *d_t = nullptr, *d_g = nullptr, *d_f = nullptr;  // images
     float *d_ua = nullptr, *d_ub = nullptr;                                  // sweep ping-pong
     float *d_imT = nullptr;                                                  // transposed image of the forward projector
+    float *d_imI = nullptr;                                                  // its interleaved copy (groups of four slices)
     float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr, *d_sw = nullptr;  // sinograms (d_sw = sqrt(w))
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
     __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
@@ -420,7 +422,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
 
 static void free_ws(tnlm_handle *H)
 {
-    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_fbp_q, &H->d_r, &H->d_rw, &H->d_q, &H->d_sw, &H->d_yh, &H->d_wh};
+    float **bufs[] = {&H->d_s, &H->d_t, &H->d_g, &H->d_f, &H->d_ua, &H->d_ub, &H->d_imT, &H->d_imI, &H->d_fbp_q, &H->d_r, &H->d_rw, &H->d_q, &H->d_sw, &H->d_yh, &H->d_wh};
     for (float **b : bufs) { if (*b) cudaFree(*b); *b = nullptr; }
     H->ws_slices = 0;
 }
@@ -508,42 +510,70 @@ struct ProfScope {
 };
 
 // ------------------------------------------------------------------------------ projector
-static int launch_transpose(tnlm_handle *H, const float *img, float *imgT, int n_slices, cudaStream_t st)
+// Which forward projector serves a call with n_slices slices, and how many of its slices (a multiple of 4, from
+// slice 0) go through the interleaved copies (interleave4_kernel, project_il_kernel, cgls_update_us_il).
+// The strip kernel issues ~1.4x the instructions of the gather kernel (staging, per-chunk extents) and has no
+// memory stalls: measured 12.7 vs 29.0 us on cfg 1 (less than one wave of work: latency bound) and 289 vs 233 us
+// on cfg 4 (issue bound).  Automatic choice: strips while the gather kernel would not fill one wave of CTAs.
+static bool use_strips(const tnlm_handle *H, int n_slices)
 {
+    const int nray = H->G.n_views * H->G.n_bins;
+    const long long gather_ctas = (long long)((nray + 255) / 256) * n_slices * H->n_phase;
+    return H->opt_project == 1 || (H->opt_project < 0 && gather_ctas < (long long)H->n_sm * 8);
+}
+static int il_slices(const tnlm_handle *H, int n_slices)
+{
+    return (H->opt_project_il && !use_strips(H, n_slices)) ? (n_slices / 4) * 4 : 0;
+}
+// The copies of img the forward projector reads: for slices [0, n_il) the two interleaved ones (d_imI, d_imT),
+// for the others the transposed image (their part of d_imT).
+static int launch_copies(tnlm_handle *H, const float *img, int n_slices, cudaStream_t st)
+{
+    int rc;
+    const int n_il = il_slices(H, n_slices);
+    if ((rc = need(H, &H->d_imT, img_count(H)))) return rc;
+    if (n_il && (rc = need(H, &H->d_imI, img_count(H)))) return rc;
     ProfScope ps(H, TNLM_KERNEL_TRANSPOSE, st);
-    dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, n_slices * H->n_phase);
-    transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(img, imgT, H->nx, H->ny);
-    LAUNCHED(H);
+    if (n_il) {
+        dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, (n_il / 4) * H->n_phase);
+        interleave4_kernel<<<tg, dim3(32, 8), 0, st>>>(img, reinterpret_cast<float4 *>(H->d_imI), reinterpret_cast<float4 *>(H->d_imT),
+                                                        H->nx, H->ny, H->n_phase);
+        LAUNCHED(H);
+    }
+    if (n_slices > n_il) {
+        dim3 tg((H->nx + 31) / 32, (H->ny + 31) / 32, (n_slices - n_il) * H->n_phase);
+        transpose_kernel<<<tg, dim3(32, 8), 0, st>>>(img, H->d_imT, H->nx, H->ny, n_il * H->n_phase);
+        LAUNCHED(H);
+    }
     return TNLM_OK;
 }
-// imgT = the transposed copy of img the shallow rays walk; NULL = make it here (d_imT).
+// copies_ready: the copies of img (launch_copies) are already in d_imI / d_imT (cgls_update_us wrote them).
 template <int MODE>
-static int launch_project(tnlm_handle *H, const float *img, const float *imgT, const float *y, const float *sw,
+static int launch_project(tnlm_handle *H, const float *img, bool copies_ready, const float *y, const float *sw,
                           float *out0, float *out1, double *red, int n_slices, cudaStream_t st)
 {
     const int nray = H->G.n_views * H->G.n_bins;
     int rc;
-    if (!imgT) {
-        if ((rc = need(H, &H->d_imT, img_count(H)))) return rc;
-        if ((rc = launch_transpose(H, img, H->d_imT, n_slices, st))) return rc;
-        imgT = H->d_imT;
-    }
+    if (!copies_ready && (rc = launch_copies(H, img, n_slices, st))) return rc;
+    const float *imgT = H->d_imT;
     ProfScope ps(H, TNLM_KERNEL_PROJECT, st);
-    // The strip kernel issues ~1.4x the instructions of the gather kernel (staging, per-chunk extents) and has no
-    // memory stalls: measured 12.7 vs 29.0 us on cfg 1 (less than one wave of work: latency bound) and 289 vs 233 us
-    // on cfg 4 (issue bound).  Automatic choice: strips while the gather kernel would not fill one wave of CTAs.
-    const long long gather_ctas = (long long)((nray + 255) / 256) * n_slices * H->n_phase;
-    const bool strips = H->opt_project == 1 || (H->opt_project < 0 && gather_ctas < (long long)H->n_sm * 8);
-    if (strips) {
+    if (use_strips(H, n_slices)) {
         const int tasks = H->G.n_views * ((H->G.n_bins + 31) / 32);
         dim3 grid((tasks + PS_WARPS - 1) / PS_WARPS, n_slices * H->n_phase);
         project_strip_kernel<MODE><<<grid, 32 * PS_WARPS, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red);
         LAUNCHED(H);
         return TNLM_OK;
     }
-    // slices of a batch share the geometry: groups of 4 (then 2, then 1) slices per thread (project_kernel)
+    const int n_il = il_slices(H, n_slices);
+    if (n_il) {                                      // groups of four slices from the interleaved copies
+        dim3 grid((nray + 255) / 256, (n_il / 4) * H->n_phase);
+        project_il_kernel<MODE><<<grid, 256, 0, st>>>(H->G, H->d_tab, H->d_rng, reinterpret_cast<const float4 *>(H->d_imI),
+                                                       reinterpret_cast<const float4 *>(H->d_imT), y, sw, out0, out1, red);
+        LAUNCHED(H);
+    }
+    // the other slices from the image and its transpose, up to project_group slices per thread (project_kernel)
     const int max_ns = H->opt_project_group;
-    int s0 = 0;
+    int s0 = n_il;
     for (int ns = 4; ns >= 1; ns >>= 1) {
         if (ns > max_ns) continue;
         const int groups = (n_slices - s0) / ns;
@@ -591,7 +621,7 @@ extern "C" int tnlm_project(tnlm_handle *H, const float *img, float *sino, int n
     int rc;
     if (!img || !sino) return fail(H, TNLM_INVALID_ARG, "img and sino must not be NULL");
     if ((rc = ensure_ws(H, n_slices))) return rc;
-    return launch_project<FWD_PLAIN>(H, img, nullptr, nullptr, nullptr, sino, nullptr, nullptr, n_slices, (cudaStream_t)stream);
+    return launch_project<FWD_PLAIN>(H, img, false, nullptr, nullptr, sino, nullptr, nullptr, n_slices, (cudaStream_t)stream);
 }
 
 extern "C" int tnlm_backproject(tnlm_handle *H, const float *sino, float *img, int n_slices, void *stream)
@@ -642,6 +672,7 @@ static int cgls_workspace(tnlm_handle *H, int m1, int n_slices, bool weighted)
     if ((rc = need(H, &H->d_s, img_count(H)))) return rc;
     if ((rc = need(H, &H->d_t, img_count(H)))) return rc;
     if ((rc = need(H, &H->d_imT, img_count(H)))) return rc;
+    if (il_slices(H, n_slices) && (rc = need(H, &H->d_imI, img_count(H)))) return rc;
     if ((rc = need(H, &H->d_r, sino_count(H)))) return rc;
     if ((rc = need(H, &H->d_rw, sino_count(H)))) return rc;
     if ((rc = need(H, &H->d_q, sino_count(H)))) return rc;
@@ -676,18 +707,29 @@ static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const 
     double *gam = H->d_scal, *qq = H->d_scal + (size_t)(m1 + 1) * nprob;
     CU(H, cudaMemsetAsync(H->d_scal, 0, (size_t)nscal * sizeof(double), st));
     float *u = g_out;
-    dim3 gs((nray + 255) / 256, nprob), gt((H->nx + 31) / 32, (H->ny + 31) / 32, nprob);
+    dim3 gs((nray + 255) / 256, nprob);
     // init (L109): r = y_n - P_n u ; s = P_n^T r ; gamma_0 = ||s||^2
-    if ((rc = launch_project<FWD_RESID>(H, u, nullptr, y, sw, H->d_r, H->d_rw, nullptr, n_slices, st))) return rc;
+    if ((rc = launch_project<FWD_RESID>(H, u, false, y, sw, H->d_r, H->d_rw, nullptr, n_slices, st))) return rc;
     if ((rc = launch_backproject(H, H->d_rw, H->d_s, gam, n_slices, st))) return rc;
-    const float *sT = nullptr;                       // transposed s: made by cgls_update_us from step 1 on
+    // Slices [0, n_il) keep s in the interleaved copies the batch projector reads (made from d_s by the first
+    // FWD_SCALE, updated in place by cgls_update_us_il); the others keep it in d_s with its transpose in d_imT.
+    const int n_il = il_slices(H, n_slices), prob_il = n_il * H->n_phase;
+    dim3 gt_il((H->nx + 31) / 32, (H->ny + 31) / 32, std::max(prob_il / 4, 1)), gt_rest((H->nx + 31) / 32, (H->ny + 31) / 32, std::max(nprob - prob_il, 1));
+    float4 *sI = reinterpret_cast<float4 *>(H->d_imI), *sTI = reinterpret_cast<float4 *>(H->d_imT);
+    bool copies_ready = false;                       // made by cgls_update_us from step 1 on
     for (int m = 0; m < m1; ++m) {
         // q = P_n s ; qq_m = ||q||^2
-        if ((rc = launch_project<FWD_SCALE>(H, H->d_s, sT, nullptr, sw, H->d_q, nullptr, qq + (size_t)m * nprob, n_slices, st))) return rc;
+        if ((rc = launch_project<FWD_SCALE>(H, H->d_s, copies_ready, nullptr, sw, H->d_q, nullptr, qq + (size_t)m * nprob, n_slices, st))) return rc;
         if (m + 1 == m1) {                           // r, t, s of the last step feed nothing (g = u^(M1), L127)
             ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
-            cgls_update_us<true><<<gt, dim3(32, 8), 0, st>>>(u, H->d_s, nullptr, nullptr, H->nx, H->ny, gam, qq, nprob, m);
-            LAUNCHED(H);
+            if (prob_il) {
+                cgls_update_us_il<true><<<gt_il, dim3(32, 8), 0, st>>>(u, sI, nullptr, nullptr, H->nx, H->ny, H->n_phase, gam, qq, nprob, m);
+                LAUNCHED(H);
+            }
+            if (nprob > prob_il) {
+                cgls_update_us<true><<<gt_rest, dim3(32, 8), 0, st>>>(u, H->d_s, nullptr, nullptr, H->nx, H->ny, gam, qq, nprob, m, prob_il);
+                LAUNCHED(H);
+            }
             break;
         }
         {
@@ -698,10 +740,16 @@ static int cgls_device(tnlm_handle *H, const float *f_in, const float *y, const 
         if ((rc = launch_backproject(H, H->d_rw, H->d_t, gam + (size_t)(m + 1) * nprob, n_slices, st))) return rc;
         {
             ProfScope ps(H, TNLM_KERNEL_CGLS_VECTOR, st);
-            cgls_update_us<false><<<gt, dim3(32, 8), 0, st>>>(u, H->d_s, H->d_t, H->d_imT, H->nx, H->ny, gam, qq, nprob, m);
-            LAUNCHED(H);
+            if (prob_il) {
+                cgls_update_us_il<false><<<gt_il, dim3(32, 8), 0, st>>>(u, sI, H->d_t, sTI, H->nx, H->ny, H->n_phase, gam, qq, nprob, m);
+                LAUNCHED(H);
+            }
+            if (nprob > prob_il) {
+                cgls_update_us<false><<<gt_rest, dim3(32, 8), 0, st>>>(u, H->d_s, H->d_t, H->d_imT, H->nx, H->ny, gam, qq, nprob, m, prob_il);
+                LAUNCHED(H);
+            }
         }
-        sT = H->d_imT;
+        copies_ready = true;
     }
     return TNLM_OK;
 }
@@ -939,6 +987,7 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
     else if (n == "apply_depth") { if ((ok = (value == 0 || value == 4 || value == 8 || value == 16))) H->opt_depth = (int)value; }
     else if (n == "apply_wpc") { if ((ok = (value == 0 || in(2, 8)))) H->opt_wpc = (int)value; }
+    else if (n == "project_interleave") { if ((ok = in(0, 1))) H->opt_project_il = (int)value; }
     else if (n == "project_group") { if ((ok = (value == 1 || value == 2 || value == 4))) H->opt_project_group = (int)value; }
     else if (n == "backproject_group") { if ((ok = (value == 1 || value == 2 || value == 4 || value == 8))) H->opt_backproject_group = (int)value; }
     else if (n == "apply_snake") { if ((ok = in(0, 1))) H->opt_snake = (int)value; }

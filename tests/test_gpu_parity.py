@@ -196,19 +196,21 @@ def test_slice_groups_share_geometry_bit_identically(T):
     w = rng.random((S, cfg.N, cfg.V, cfg.B)) * 50 + 1
     imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
     ref = {}
-    for pg, bg in [(1, 1), (2, 2), (4, 4), (4, 8), (1, 8)]:
+    # project_interleave: slices 0..7 through the interleaved copies (project_il_kernel, cgls_update_us_il), 8..10 not
+    for pg, bg, il in [(1, 1, 0), (2, 2, 0), (4, 4, 0), (4, 8, 1), (1, 8, 1), (2, 1, 1)]:
         tn.set_option(hd, "project_kernel", 0); tn.set_option(hd, "project_group", pg); tn.set_option(hd, "backproject_group", bg)
+        tn.set_option(hd, "project_interleave", il)
         po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
         tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo)
-        tn.cgls_step(hd, imgd, sinod, wd, 2, go)          # fused epilogues and per-problem reductions of every slice
+        tn.cgls_step(hd, imgd, sinod, wd, 3, go)          # fused epilogues and per-problem reductions of every slice
         if not ref:
             ref = dict(p=po, b=bo, g=go)
             for s in (0, 7, 8, 10):
                 assert rel(po[s].cpu().numpy(), oracle.project(og, img[s])) < 2e-6
                 assert rel(bo[s].cpu().numpy(), oracle.backproject(og, sino[s], cfg.L, cfg.L)) < 2e-6
-                assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 2)) < STEP_TOL
+                assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 3)) < STEP_TOL
         else:
-            assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg)
+            assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg, il)
 
 
 @pytest.mark.parametrize("B,V", [(120, 16), (200, 9)], ids=["fan76", "fan127"])
