@@ -451,7 +451,9 @@ def recon_kernel_entries(cfg, n_slices, table, total_us, peak_tf, hbm_gbs):
             e.update({"bound": "alu", "algorithmic_tflops": fl / sec / 1e12, "algorithmic_gbs": 12.0 * n_img / sec / 1e9,
                       "frac_symmetric_flop_count": flops_per_px_update_symmetric(cfg.window, cfg.patch) * n_img / sec / 1e12 / peak_tf})
         elif kind == "transpose":
-            e.update({"bound": "hbm", "algorithmic_gbs": 8.0 * n_img / sec / 1e9})
+            # the copies the forward projector reads: one transposed image (read 4 B, write 4 B per pixel), or, for
+            # groups of four slices of a batch, the two interleaved copies (read 4 B, write 8 B per pixel)
+            e.update({"bound": "hbm", "algorithmic_gbs": (12.0 if n_slices >= 4 else 8.0) * n_img / sec / 1e9})
         elif kind == "cgls_vector":
             # mean over its launches: r update (16 B per ray), fused u/s update (28 B per pixel), last u update (12 B)
             e.update({"bound": "hbm", "algorithmic_gbs": None})
