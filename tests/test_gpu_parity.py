@@ -590,6 +590,34 @@ def test_multi_slice_reconstruct_and_host_entry_points(T):
     assert torch.equal(fo, od.cpu())
 
 
+def test_batch_reconstruct_equals_per_slice_reconstruct(T):
+    # A batch runs its projectors on groups of slices (8 per thread in the backprojector, 4 interleaved per pixel
+    # in the forward projector, the rest one by one); a single slice takes the single-slice kernels.  The slices
+    # are independent and the per-slice arithmetic is the same: S = 9 (two forward groups + 1, one
+    # backprojector group + 1) reconstructed in one call equals nine single-slice calls bit for bit, whether or
+    # not the handle grew its workspace in between, and a group-sized batch (S = 4, S = 8) has no remainder path.
+    # (The sweep's launch shape is pinned: the cost model picks it from the number of images, and the vertical
+    # running sums of a band round differently when the band starts on another row -- last-bit differences.)
+    torch, tn = T
+    cfg = workloads.config(1, S=9, seed=6)
+    inp = workloads.make_inputs(cfg)
+    h, og = handles(tn, cfg)
+    tn.set_option(h, "sweep_rb", 8); tn.set_option(h, "sweep_nb", 2)
+    y, w = dev(torch, inp["y"]), dev(torch, inp["w"])
+    out = torch.empty(cfg.S, cfg.N, cfg.L, cfg.L, device="cuda")
+    tn.reconstruct(h, y, w, None, 2, 3, 1, out)
+    for s in range(cfg.S):
+        one = torch.empty(1, cfg.N, cfg.L, cfg.L, device="cuda")
+        tn.reconstruct(h, y[s:s + 1].contiguous(), w[s:s + 1].contiguous(), None, 2, 3, 1, one)
+        assert torch.equal(one[0], out[s]), s
+    for S in (4, 8):
+        part = torch.empty(S, cfg.N, cfg.L, cfg.L, device="cuda")
+        tn.reconstruct(h, y[:S].contiguous(), w[:S].contiguous(), None, 2, 3, 1, part)
+        assert torch.equal(part, out[:S]), S
+    want = oracle.reconstruct(og, inp["y"][8], inp["w"][8], None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 2, 3, 1)
+    assert rel(out[8].cpu().numpy(), want) < STEP_TOL * 5
+
+
 def test_config4_size_cgls_and_reconstruct_match_oracle(T):
     # BASELINE config 4 at full size (512^2 x 10, 60 views x 888 bins, W=15, d=7, h=0.005: the sharpest
     # softmax of the configs), every pixel: three CGLS steps from a noisy start, then three outer
