@@ -9,6 +9,8 @@
 //   backproject_kernel          t = P^T rw, gamma_{m+1}
 //   cgls_update_us              u += a_m s_m ; s_{m+1} = t + b_m s_m ; sT = s_{m+1}^T   (one image pass)
 // The last step only needs u += a_m s_m (cgls_update_us<true>): r, t, s of step M1 feed nothing (L127).
+// In a call with four or more slices the groups of four slices run project_il_kernel / cgls_update_us_il instead:
+// their s lives only in the interleaved copies the batch projector reads (projector.cuh).
 #pragma once
 #include "common.cuh"
 
