@@ -434,7 +434,12 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     for (cudaEvent_t e : H->prof_ev) cudaEventDestroy(e);
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
-    if (H->d_wts) cudaFree(H->d_wts);
+    if (H->d_wts) {
+        cudaFree(H->d_wts);
+        // the evict_last lines of the stored weights (apply_resident_mb) would otherwise keep their L2 priority
+        // until something else claims it; ignore a driver that does not support the call
+        if (cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
+    }
     if (H->d_fbp_g) cudaFree(H->d_fbp_g);
     if (H->d_fbp_cosw) cudaFree(H->d_fbp_cosw);
     if (H->d_fbp_wv) cudaFree(H->d_fbp_wv);
@@ -905,7 +910,12 @@ static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_s
     const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
     if (H->opt_cache_mb <= 0 || need * sizeof(__nv_bfloat16) > (size_t)H->opt_cache_mb * 1048576ull) return nullptr;
     if (need > H->wts_cap) {
-        if (H->d_wts) cudaFree(H->d_wts);
+        if (H->d_wts) {
+        cudaFree(H->d_wts);
+        // the evict_last lines of the stored weights (apply_resident_mb) would otherwise keep their L2 priority
+        // until something else claims it; ignore a driver that does not support the call
+        if (cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
+    }
         H->d_wts = nullptr; H->wts_cap = 0;
         if (cudaMalloc(&H->d_wts, need * sizeof(__nv_bfloat16)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
         H->wts_cap = need;
