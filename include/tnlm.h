@@ -177,7 +177,9 @@ int tnlm_device(const tnlm_handle *handle);
 /* Per-launch device timing of every kernel of the path, for benchmarks and rooflines.
  * tnlm_profile_kernels(handle, 1) makes every later call bracket each kernel launch with a CUDA
  * event pair on the call's stream (0 switches it off; either call forgets the launches recorded
- * so far).  tnlm_kernel_times waits for the recorded launches, writes up to `capacity` durations
+ * so far).  One pair covers one operation on the whole batch: a projector application whose slices
+ * run as several group sizes (say 8 + 2 + 1 slices per thread) is a few back-to-back launches inside
+ * one pair.  tnlm_kernel_times waits for the recorded launches, writes up to `capacity` durations
  * (milliseconds, launch order) into the HOST arrays ms[] and kind[] (a tnlm_kernel_kind), stores
  * the number recorded in *count, and forgets them. */
 typedef enum {
@@ -186,7 +188,7 @@ typedef enum {
     TNLM_KERNEL_APPLY = 2,       /* one Gauss-Jacobi sweep of Eq. (7) from the stored weights */
     TNLM_KERNEL_PROJECT = 3,     /* forward projector P with the CGLS epilogue (L75, L109, L112) */
     TNLM_KERNEL_BACKPROJECT = 4, /* backprojector P^T with the norm reduction (L79, L109, L124) */
-    TNLM_KERNEL_TRANSPOSE = 5,   /* transposed image copy read by the shallow rays of P */
+    TNLM_KERNEL_TRANSPOSE = 5,   /* the image copies P reads: transposed (shallow rays) or, in a batch, four slices interleaved */
     TNLM_KERNEL_CGLS_VECTOR = 6, /* CGLS vector updates (L114-L126) and sqrt(w) */
     TNLM_KERNEL_CLIP = 7,        /* positivity clip alone (m2 = 0) */
     TNLM_KERNEL_FBP = 8          /* FBP initialisation kernels (L175) */
