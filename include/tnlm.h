@@ -92,7 +92,8 @@ typedef enum {
     TNLM_CUDA_ERROR = 2,  /* a CUDA runtime call failed; message from cudaGetErrorString */
     TNLM_ALLOC_FAILED = 3,
     TNLM_UNSUPPORTED = 4  /* device is not sm_100, patch/window above the compiled maximum
-                             (patch <= 9, window <= 31), flat detector */
+                             (patch <= 9, window <= 31), flat detector, a fan of 180 degrees or more,
+                             a source closer than six pixels to the circle around the image */
 } tnlm_status;
 
 typedef struct tnlm_handle tnlm_handle; /* opaque: geometry tables + workspace */

@@ -297,6 +297,8 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         if (!g.detector_arc) return fail(nullptr, TNLM_UNSUPPORTED, "flat detector not built; the paper's detector is an arc");
         const double hx = 0.5 * nx * g.pixel_mm, hy = 0.5 * ny * g.pixel_mm;
         if (std::sqrt(hx * hx + hy * hy) >= g.sid_mm) return fail(nullptr, TNLM_INVALID_ARG, "geometry: image corner outside the source circle");
+        if (g.sid_mm - std::sqrt(hx * hx + hy * hy) < 6.0 * g.pixel_mm)
+            return fail(nullptr, TNLM_UNSUPPORTED, "geometry: source closer than six pixels to the image (the backprojector's candidate ranges assume at least that)");
         if ((long long)g.n_views * g.n_bins > 2000000000LL) return fail(nullptr, TNLM_UNSUPPORTED, "sinogram too large");
     }
     int dev = 0;

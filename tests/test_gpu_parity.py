@@ -213,8 +213,9 @@ def test_slice_groups_share_geometry_bit_identically(T):
             assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg, il)
 
 
-@pytest.mark.parametrize("B,V", [(120, 16), (200, 9)], ids=["fan76", "fan127"])
-def test_backprojector_candidate_range_misses_no_ray(T, B, V):
+@pytest.mark.parametrize("B,V,L,sid", [(120, 16, 40, 45.0), (200, 9, 40, 45.0), (66, 40, 6, 14.6), (90, 12, 12, 15.0), (140, 7, 30, 27.5)],
+                         ids=["fan76", "fan127", "near6", "near12", "near30"])
+def test_backprojector_candidate_range_misses_no_ray(T, B, V, L, sid):
     # The gather's candidate bins per (2 x 2 block, view) are a conservative range around the block centre's fan
     # angle; a range one bin too narrow would drop matrix entries silently.  On a mid-size geometry with a wide fan and
     # a near source (large, direction-dependent angular footprints) every entry of P^T must equal P's, bit for bit:
@@ -222,7 +223,9 @@ def test_backprojector_candidate_range_misses_no_ray(T, B, V):
     torch, tn = T
     # (B = 200: a 127-degree fan, so a view's bins change between steep and shallow twice: three runs in the
     # backprojector's per-view run table)
-    cfg = workloads.Config("wide", L=40, N=1, V=V, B=B, pitch=1.0, sid=45.0, sdd=90.0, window=3, patch=3)
+    # (near*: a source 6-10 pixels from the circle around the image, where a block's angular footprint changes by
+    # 10-25 % across its own candidate range: found by random-geometry fuzzing, not by the configs)
+    cfg = workloads.Config("wide", L=L, N=1, V=V, B=B, pitch=0.7 if L < 40 else 1.0, sid=sid, sdd=2.0 * sid, window=3, patch=3)
     h, og = handles(tn, cfg)
     npx, nr = cfg.L * cfg.L, cfg.V * cfg.B
     eye = torch.eye(npx, device="cuda").view(npx, 1, cfg.L, cfg.L)
@@ -236,6 +239,51 @@ def test_backprojector_candidate_range_misses_no_ray(T, B, V):
         row = torch.empty(npx, device="cuda")
         tn.backproject(h, e.view(1, cfg.V, cfg.B), row.view(1, cfg.L, cfg.L))
         assert torch.equal(row, cols[:, q].contiguous()), int(q)
+
+# ------------------------------------------------------------------------------- random shapes
+def test_random_shapes_match_oracle(T):
+    # Seeded random shapes and parameters (image sizes with ragged tiles, every window / patch size, one to three
+    # slices; random fan-beam geometries from near sources and wide fans to far sources, one to eleven slices so that
+    # every slice-group size of the batch projectors occurs), each compared with the oracle.  A longer run of the
+    # same generator is how the near-source candidate-range bug of the backprojector was found.  Bins are even in
+    # number and the source stays six pixels off the image circle: an odd number of bins puts the central ray of an
+    # axis-aligned view exactly on a grid line of an even-sized image (reading 16).
+    torch, tn = T
+    rng = np.random.default_rng(20261104)
+    f32 = lambda a: a.astype(np.float32).astype(np.float64)
+    for _ in range(24):
+        N = int(rng.integers(1, 6)); ny = int(rng.integers(3, 100)); nx = int(rng.integers(3, 300))
+        W = int(rng.choice([1, 3, 5, 7, 9, 11, 13, 15, 21, 31])); d = int(rng.choice([1, 3, 5, 7, 9]))
+        h = float(rng.choice([0.002, 0.005, 0.01, 0.05, 1.0])); mu = float(rng.choice([0.0, 0.05, 0.3, 2.0]))
+        m2 = int(rng.integers(1, 5)); S = int(rng.integers(1, 4))
+        if ny * nx * N * S * W * W * d * d > 1.5e9:
+            continue
+        g = rng.random((S, N, 1, 1)) * 0.02 + rng.normal(0, 0.002, (S, N, ny, nx)) + 0.01 * (rng.random((S, 1, ny, nx)) > 0.7)
+        hd = tn.create(None, nx, ny, N, W, d, h, mu)
+        out = torch.empty(S, N, ny, nx, device="cuda")
+        tn.regularize_step(hd, dev(torch, g), m2, out)
+        want = np.stack([oracle.regularize_step(f32(g[s]), W, d, h, mu, m2) for s in range(S)])
+        assert rel(out.cpu().numpy(), want) < STEP_TOL, (N, ny, nx, W, d, h, mu, m2, S)
+        hd.close()
+    for _ in range(24):
+        L = int(rng.integers(5, 70)); N = int(rng.integers(1, 4)); V = int(rng.integers(3, 50)); B = 2 * int(rng.integers(4, 70))
+        S = int(rng.integers(1, 12)); m1 = int(rng.integers(0, 4))
+        sid = float(L * rng.uniform(0.7072, 3.0)) + 6.01; sdd = sid * float(rng.uniform(1.2, 2.0)); pitch = float(rng.uniform(0.5, 2.0))
+        cfg = workloads.Config("random", L=L, N=N, V=V, B=B, pitch=pitch, sid=sid, sdd=sdd, I0=1e4, window=3, patch=3, h=0.01, mu=0.1)
+        try:
+            hd, og = handles(tn, cfg)
+        except tn.TnlmError:               # a fan of 180 degrees or more: refused, not wrong
+            continue
+        img = rng.random((S, N, L, L)) * 0.02; sino = rng.random((S, N, V, B)); w = rng.random((S, N, V, B)) * 50 + 1
+        imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
+        po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
+        tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo); tn.cgls_step(hd, imgd, sinod, wd, m1, go)
+        s = int(rng.integers(0, S))
+        key = (L, N, V, B, S, m1, sid, sdd, pitch)
+        assert rel(po[s].cpu().numpy(), oracle.project(og, f32(img[s]))) < 1e-5, key
+        assert rel(bo[s].cpu().numpy(), oracle.backproject(og, f32(sino[s]), L, L)) < 1e-5, key
+        assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, f32(img[s]), f32(sino[s]), f32(w[s]), m1)) < STEP_TOL, key
+        hd.close()
 
 
 # ------------------------------------------------------------------------------------- CGLS
