@@ -28,7 +28,7 @@ struct Geom {
     float pix;                 // mm
     float sdd_over_pitch;      // bins per radian of fan angle
     float bin_centre;          // (B-1)/2 - bin_offset
-    float hw_scale;            // 1.02 * pix * sdd_over_pitch: half-side of a 2 x 2 pixel block in bins x distance
+    float hw_scale;            // 1.02 * widening * pix * sdd_over_pitch (tnlm_create): candidate half-width of the backprojector per pixel of half-side
 };
 
 // floor() of |x| < 2^22 without the conversion unit: round-down add of 1.5*2^23 leaves floor(x)

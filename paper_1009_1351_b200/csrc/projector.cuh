@@ -542,15 +542,11 @@ backproject_kernel(Geom G, const RayEntry *__restrict__ tab, const float4 *__res
             // a ray at angle D from the direction of the block centre (distance d) crosses the block (half-sides
             // hx = BC/2, hy = BR/2 pixels, half-diagonal hd) iff d*|sin D| <= h(n) = pix*(hx*|nx| + hy*|ny|), n the
             // ray's unit normal; n turns with D, |h(n) - h(n0)| <= hd*|D| with n0 = (-py, px)/d, so
-            // |D| <= (h(n0)/d) / (1 - hd/d) up to the sinc term: h(n0)/d = pix*(hx*|py| + hy*|px|)/d^2 <= .../dot^2
-            // (hw_scale carries pix, bins per radian and 2 % for the second-order terms), widened by
-            // 1/(1 - s) <= 1 + s + 2 s^2 with s = hd/dot <= 0.25 (tnlm_create keeps the source six pixels away from
-            // the image: without this factor a source ~15 pixels from the image lost matrix entries), + 0.05 bin
-            // of rounding
-            constexpr float HD = 0.5f * 1.4142136f * (float)(BR > BC ? BR : BC);      // >= half-diagonal in pixels
-            const float sn = G.pix * HD * rdot;
-            const float hw = fmaf(G.hw_scale * (0.5f * (float)BC * fabsf(py) + 0.5f * (float)BR * fabsf(px)) * (rdot * rdot),
-                                  fmaf(sn, fmaf(2.0f, sn, 1.0f), 1.0f), 0.05f);
+            // |D| <= (h(n0)/d) / (1 - hd/d) up to the sinc term: h(n0)/d = pix*(hx*|py| + hy*|px|)/d^2 <= .../dot^2.
+            // hw_scale carries pix, bins per radian, 2 % for the second-order terms and the factor 1/(1 - hd/d) at
+            // the smallest d of the geometry (tnlm_create: without it a source ~15 pixels from the image lost matrix
+            // entries; found by random-geometry fuzzing), + 0.05 bin of rounding
+            const float hw = fmaf(G.hw_scale * (0.5f * (float)BC * fabsf(py) + 0.5f * (float)BR * fabsf(px)), rdot * rdot, 0.05f);
             const int k_lo = max(0, __float_as_int(__fadd_ru(kc - hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             const int k_hi = min(B - 1, __float_as_int(__fadd_rd(kc + hw, FLOOR_MAGIC)) - FLOOR_MAGIC_BITS);
             // the steep / shallow classes are contiguous runs of the bin index (a fan narrower than 90 degrees crosses a

@@ -362,7 +362,13 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
             const double rmax = std::sqrt(hx * hx + hy * hy) + g.pixel_mm;
             H->fan_poly = rmax / std::sqrt(std::fmax(g.sid_mm * g.sid_mm - rmax * rmax, 1e-30)) < 0.95;
         }
-        G.hw_scale = (float)(1.02 * g.pixel_mm * g.sdd_mm / g.bin_pitch_mm);    // x pixels of half-side
+        {   // backproject_kernel's candidate half-width (see there): pix x bins per radian x 1.02 x 1/(1 - s), s = the
+            // half-diagonal of a 2 x 2 pixel block over the smallest distance of a block centre from the source
+            // plane (>= sid - image half-diagonal >= 6 pixels, checked above), 1/(1 - s) <= 1 + s + 2 s^2 for s <= 1/2
+            const double hxm = 0.5 * nx * g.pixel_mm, hym = 0.5 * ny * g.pixel_mm;
+            const double sn = 1.4143 * g.pixel_mm / (g.sid_mm - std::sqrt(hxm * hxm + hym * hym));
+            G.hw_scale = (float)(1.02 * (1.0 + sn + 2.0 * sn * sn) * g.pixel_mm * g.sdd_mm / g.bin_pitch_mm);
+        }
         std::vector<RayEntry> tab; std::vector<RayRange> rng; std::vector<float4> views; std::vector<int4> split;
         if (!build_tables(g, nx, ny, n_phase, tab, rng, views, split)) {
             tnlm_destroy(H);
