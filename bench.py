@@ -8,7 +8,7 @@ N=1: BASELINE.json configs[1] ("TNLM step alone": 256x256 fp32 x 10 cyclic phase
 patch 5, h=0.008, mu=0.1, 10 Gauss-Jacobi sweeps, seed 1).  One step = one
 tnlm_regularize_step call (weights + 10 sweeps + clip) on one slice per GPU: 1 launch of
 gj_sweep_kernel<.,.,true> (weights of g in fp32, sweep 1, stores the weights as bf16) and 9
-launches of gj_apply2_kernel (sweeps 2..10 from the stored weights, fp32 accumulation, HBM bound).
+launches of gj_apply3_kernel (sweeps 2..10 from the stored weights, fp32 accumulation, HBM bound).
 
 --gpus N > 1: when not already under torchrun, bench.py re-executes itself under
 `python -m torch.distributed.run --nproc-per-node N` (one rank per GPU, NCCL for the barrier and
@@ -371,7 +371,7 @@ def run_ours(args):
             traffic = {}
     names = {"sweep": "gj_sweep_kernel<PB,RB,false> (weights on the fly + sweep)",
              "sweep_store": "gj_sweep_kernel<PB,RB,true> (weights on the fly + sweep, stores bf16 weights)",
-             "apply": "gj_apply2_kernel (sweep from stored bf16 weights, persistent warp tasks)"}
+             "apply": "gj_apply3_kernel (sweep from stored bf16 weights: one CTA per band, per-warp cp.async rings)"}
 
     def tnlm_entry(kind, per_step, us, step_us_):
         k = {"kernel": names[kind], "launches_per_step": per_step, "us_per_launch": us,

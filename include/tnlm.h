@@ -61,8 +61,9 @@
  *   recompute the weights in fp32), sweep_rb, sweep_nb / TNLM_SWEEP_SHAPE="rb,nb" and
  *   apply_ns / TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).  Options without an
  *   environment variable (kernel variants kept for comparison; results are bit-identical either way):
- *   apply_kernel (1 = persistent warp-task stored-weight sweep, the default; 0 = one CTA per band with a TMA
- *   ring), apply_depth, apply_wpc (ring depth and warps per CTA of the former; 0 = cost model),
+ *   apply_kernel (2 = one CTA per stored band, both windows shared, one cp.async ring per warp: the default;
+ *   1 = persistent warp tasks with private windows; 0 = one CTA per band with a TMA ring), apply_depth (ring depth of
+ *   kernels 1 and 2; 0 = chosen by the library), apply_wpc (warps per CTA of kernel 1; 0 = cost model),
  *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers),
  *   apply_snake (1, the default: successive stored-weight sweeps deal their tasks in opposite orders, so a sweep
  *   starts on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored

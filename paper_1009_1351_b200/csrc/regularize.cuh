@@ -785,6 +785,135 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     }
 }
 
+// The same sweep with one CTA per stored band (chunk): its rb/2 warps (one per row pair) share the u_j windows of
+// BOTH sides (rb + 2a rows each, staged once by all threads), so a warp's 2 W^2 pieces form one uninterrupted
+// stream -- gj_apply2_kernel drains its ring and restages a window between the two sides of every task (two pipeline
+// restarts of ~2.5 us in a 62 us launch, and 3x the window bytes from L2).  Arithmetic and its order are those of
+// gj_apply2_kernel (bit-identical results).  grid.x = chunks = (S*N) * bands that hold image rows * tiles_x;
+// block = 32 * rb/2; dynamic smem = apply3_smem_bytes.
+__host__ __device__ inline size_t apply3_smem_bytes(int window, int rb, int depth)
+{
+    const int a = (window - 1) / 2;
+    return (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) + (size_t)(rb / 2) * depth * 512;
+}
+
+template <int DEPTH>             // pieces in flight per warp (a power of two)
+__global__ void __launch_bounds__(160, 4)
+gj_apply3_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
+                 const __nv_bfloat16 *__restrict__ wts)
+{
+    constexpr int C = SW_C;
+    const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1, WW = W * W;
+    const int rb = p.rb, npairs = rb >> 1, urows = rb + 2 * a, UW = apply_uw(W);
+    const size_t pstride = (size_t)rb * (SW_TW / 8);     // uint4 per offset plane
+    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)WW * pstride;      // uint4
+    const size_t npix = (size_t)nx * ny;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    extern __shared__ float4 smem4[];
+    float *sU = reinterpret_cast<float *>(smem4);                                            // [2][urows][UW]
+    const unsigned ring_s = smem_u32(sU + 2 * urows * UW) + warp * (DEPTH * 512) + 16 * lane; // [npairs][DEPTH][32] x 16 B
+
+    const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
+    const long long n_chunks = (long long)p.n_img * tiles_per_img;
+    const long long chunk = p.ap_reverse ? n_chunks - 1 - (long long)blockIdx.x : (long long)blockIdx.x;
+    const int img = (int)(chunk / tiles_per_img);
+    const int tl = (int)(chunk - (long long)img * tiles_per_img);
+    const int gband = tl / p.tiles_x, tx = tl - gband * p.tiles_x;
+    const int tile_r0 = gband * rb, tile_c0 = tx * SW_TW, c0 = tile_c0 + C * lane;
+    const int r = tile_r0 + 2 * warp;
+    const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
+    const uint64_t pol = chunk * npairs < p.res_tasks ? l2_policy_evict_last() : l2_policy_evict_first();
+
+    // oldest group: both windows (all threads of the CTA)
+#pragma unroll
+    for (int sd = 0; sd < 2; ++sd) {
+        const int j = (phase + (sd == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
+        stage_tile_async(sU + sd * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a, tile_c0 - a,
+                         ny, nx, warp, npairs, lane);
+    }
+    cp_async_commit();
+    // this warp's pieces: 0 .. WW-1 of side 0, then WW .. 2 WW-1 of side 1, one stream
+    const uint4 *__restrict__ ws0 = reinterpret_cast<const uint4 *>(wts) +
+                                    ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)WW * pstride + warp * 32 + lane;
+    const uint4 *__restrict__ ws1 = ws0 + side_stride;
+    const uint4 *__restrict__ nextp = ws0;
+    unsigned issued = 0, wr = ring_s;
+    const unsigned total = 2u * (unsigned)WW;
+#pragma unroll 1
+    for (; issued < DEPTH - 1; ++issued) {
+        cp_async16_s_hint(wr, nextp, issued < total, pol);
+        cp_async_commit();
+        wr += 512;
+        nextp = (issued + 1 == (unsigned)WW) ? ws1 : nextp + pstride;
+    }
+    cp_async_wait<DEPTH - 1>();                               // this thread's window copies have landed
+    __syncthreads();                                          // ... and everybody else's
+    float nbsum[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+    unsigned t = 0;
+#pragma unroll 1
+    for (int sd = 0; sd < 2; ++sd) {
+        float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+        const float *__restrict__ uwin = sU + (sd * urows + 2 * warp) * UW + C * lane;
+#pragma unroll 1
+        for (int dr = 0; dr < W; ++dr) {
+            const float *__restrict__ urow0 = uwin + dr * UW;
+#pragma unroll 1
+            for (int k = 0; k < W; k += 4) {
+                const float4 ua = *reinterpret_cast<const float4 *>(urow0 + k), ub = *reinterpret_cast<const float4 *>(urow0 + k + 4);
+                const float4 uc = *reinterpret_cast<const float4 *>(urow0 + UW + k), ud = *reinterpret_cast<const float4 *>(urow0 + UW + k + 4);
+                const float uw0[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
+                const float uw1[8] = {uc.x, uc.y, uc.z, uc.w, ud.x, ud.y, ud.z, ud.w};
+                const int noff = min(4, W - k);
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    if (jj < noff) {
+                        cp_async16_s_hint(wr, nextp, issued < total, pol);
+                        cp_async_commit();                    // (empty groups keep the wait count uniform)
+                        ++issued;
+                        nextp = (issued == (unsigned)WW) ? ws1 : nextp + pstride;
+                        wr = (wr == ring_s + (DEPTH - 1) * 512) ? ring_s : wr + 512;
+                        cp_async_wait<DEPTH - 1>();           // piece t has landed (this lane's own 16 bytes)
+                        const uint4 wv = lds128_s(ring_s + ((t & (DEPTH - 1)) << 9));
+                        ++t;
+                        const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
+                                             __uint_as_float(wv.y << 16), __uint_as_float(wv.y & 0xffff0000u)};
+                        const float w1[C] = {__uint_as_float(wv.z << 16), __uint_as_float(wv.z & 0xffff0000u),
+                                             __uint_as_float(wv.w << 16), __uint_as_float(wv.w & 0xffff0000u)};
+#pragma unroll
+                        for (int c = 0; c < C; ++c) {
+                            Z[0][c] += w0[c];
+                            A[0][c] = fmaf(w0[c], uw0[c + jj], A[0][c]);
+                            Z[1][c] += w1[c];
+                            A[1][c] = fmaf(w1[c], uw1[c + jj], A[1][c]);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+            nbsum[0][c] += A[0][c] / Z[0][c];
+            nbsum[1][c] += A[1][c] / Z[1][c];
+        }
+    }
+    if (c0 < nx) {
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            if (r + q < ny) {
+                const float *__restrict__ gi = g + (size_t)img * npix + (size_t)(r + q) * nx + c0;
+                float *__restrict__ o = out + (size_t)img * npix + (size_t)(r + q) * nx + c0;
+#pragma unroll
+                for (int c = 0; c < C; ++c)
+                    if (c0 + c < nx) {
+                        float v = fmaf(p.c_nb, nbsum[q][c], p.c_self * __ldg(gi + c));
+                        if (p.clip) v = fmaxf(v, 0.f);
+                        o[c] = v;
+                    }
+            }
+        }
+    }
+}
+
 // f = max(g, 0): the m2 = 0 case of steps 3-5.
 __global__ void clip_kernel(const float *__restrict__ g, float *__restrict__ out, size_t n)
 {

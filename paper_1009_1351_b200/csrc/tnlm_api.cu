@@ -46,7 +46,8 @@ struct tnlm_handle {
     long long opt_cache_mb = 16384;
     int opt_rb = 0, opt_nb = 0, opt_ns = 0;
     int opt_project = -1;   // 1: project_strip_kernel (shared-memory strips per warp); 0: project_kernel (L1 gathers); -1: by size
-    int opt_apply = 1;      // 1: gj_apply2_kernel (persistent warp tasks, cp.async rings); 0: gj_apply_kernel (TMA ring)
+    int opt_apply = 2;      // 2: gj_apply3_kernel (CTA per band, shared windows, per-warp cp.async rings); 1: gj_apply2_kernel
+                            // (persistent warp tasks); 0: gj_apply_kernel (CTA per band, TMA ring)
     int opt_depth = 0;      // gj_apply2_kernel ring depth override (0 = cost model)
     int opt_wpc = 0;        // gj_apply2_kernel warps per CTA override (0 = cost model)
     int opt_project_il = 1;         // forward projector: groups of four slices read interleaved copies (project_il_kernel)
@@ -338,7 +339,8 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         if (ce == cudaSuccess)
             ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
                                       cudaSharedmemCarveoutMaxShared);
-        for (const void *fn : {(const void *)gj_apply2_kernel<4>, (const void *)gj_apply2_kernel<8>, (const void *)gj_apply2_kernel<16>})
+        for (const void *fn : {(const void *)gj_apply2_kernel<4>, (const void *)gj_apply2_kernel<8>, (const void *)gj_apply2_kernel<16>,
+                               (const void *)gj_apply3_kernel<4>, (const void *)gj_apply3_kernel<8>, (const void *)gj_apply3_kernel<16>})
             if (ce == cudaSuccess) ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)H->apply_smem);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
     }
@@ -846,6 +848,23 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
+    if (H->opt_apply == 2) {
+        // one CTA per band, the windows of both sides shared by its warps (gj_apply3_kernel)
+        R.n_img = n_slices * H->n_phase;
+        int dp = H->opt_depth ? H->opt_depth : 8;
+        while (dp > 4 && apply3_smem_bytes(H->window, sh.rb, dp) > H->apply_smem) dp >>= 1;
+        const size_t sm = apply3_smem_bytes(H->window, sh.rb, dp);
+        if (sm > H->apply_smem) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+        const unsigned threads = 32u * (unsigned)(sh.rb / 2);
+        ProfScope ps(H, TNLM_KERNEL_APPLY, st);
+        switch (dp) {
+            case 16: gj_apply3_kernel<16><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+            case 8: gj_apply3_kernel<8><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+            default: gj_apply3_kernel<4><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+        }
+        LAUNCHED(H);
+        return TNLM_OK;
+    }
     if (H->opt_apply == 1) {
         // Persistent warp tasks (row pairs).  Launch shape by a small cost model: for every ring depth and CTA
         // size, the resident warps W and the bytes they keep in flight bound the rate of a round at
@@ -1001,7 +1020,7 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "sweep_rb") H->opt_rb = (int)value;
     else if (n == "sweep_nb") H->opt_nb = (int)value;
     else if (n == "apply_ns") { if ((ok = in(0, AP_NS_MAX))) H->opt_ns = (int)value; }
-    else if (n == "apply_kernel") { if ((ok = in(0, 1))) H->opt_apply = (int)value; }
+    else if (n == "apply_kernel") { if ((ok = in(0, 2))) H->opt_apply = (int)value; }
     else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
     else if (n == "apply_depth") { if ((ok = (value == 0 || value == 4 || value == 8 || value == 16))) H->opt_depth = (int)value; }
     else if (n == "apply_wpc") { if ((ok = (value == 0 || in(2, 8)))) H->opt_wpc = (int)value; }

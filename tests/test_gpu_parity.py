@@ -404,7 +404,8 @@ def test_stored_weights_equal_recomputed_weights(T):
 
 
 def test_both_stored_weight_sweep_kernels_agree(T):
-    # gj_apply2_kernel (default: persistent warp tasks, cp.async rings, every ring depth and CTA size the cost model
+    # gj_apply3_kernel (default: one CTA per band, windows shared, per-warp cp.async rings), gj_apply2_kernel (option
+    # apply_kernel = 1: persistent warp tasks, cp.async rings, every ring depth and CTA size the cost model
     # may pick) and gj_apply_kernel (option apply_kernel = 0: one CTA per band, TMA ring) read the same stored layout
     # and accumulate in the same order: bit-identical results; both match the oracle.
     torch, tn = T
@@ -416,6 +417,11 @@ def test_both_stored_weight_sweep_kernels_agree(T):
         tn.set_option(hd, "apply_kernel", 0)
         tn.regularize_step(hd, gd, m2, ref)
         assert rel(ref.cpu().numpy(), oracle.regularize_step(g, W, d, h, mu, m2)) < STEP_TOL
+        for depth in (0, 4, 16):                 # gj_apply3_kernel: one CTA per band, both windows shared by its warps
+            tn.set_option(hd, "apply_kernel", 2); tn.set_option(hd, "apply_depth", depth)
+            out = torch.empty_like(gd)
+            tn.regularize_step(hd, gd, m2, out)
+            assert torch.equal(out, ref), (W, "apply3", depth)
         tn.set_option(hd, "apply_kernel", 1)
         for depth, wpc in [(0, 0), (4, 2), (8, 3), (16, 8), (8, 6)]:
             tn.set_option(hd, "apply_depth", depth); tn.set_option(hd, "apply_wpc", wpc)
@@ -424,11 +430,13 @@ def test_both_stored_weight_sweep_kernels_agree(T):
             assert torch.equal(out, ref), (W, depth, wpc)
         # task order (snake over the sweeps) and L2 residency hints change where bytes come from, not one bit
         tn.set_option(hd, "apply_depth", 0); tn.set_option(hd, "apply_wpc", 0)
-        for snake, mb in [(0, 0), (1, 0), (0, 1), (1, 1), (1, 4096)]:
-            tn.set_option(hd, "apply_snake", snake); tn.set_option(hd, "apply_resident_mb", mb)
-            out = torch.empty_like(gd)
-            tn.regularize_step(hd, gd, m2, out)
-            assert torch.equal(out, ref), (W, snake, mb)
+        for kern in (1, 2):
+            tn.set_option(hd, "apply_kernel", kern)
+            for snake, mb in [(0, 0), (1, 0), (0, 1), (1, 1), (1, 4096)]:
+                tn.set_option(hd, "apply_snake", snake); tn.set_option(hd, "apply_resident_mb", mb)
+                out = torch.empty_like(gd)
+                tn.regularize_step(hd, gd, m2, out)
+                assert torch.equal(out, ref), (W, kern, snake, mb)
 
 
 def test_regularize_multi_slice_equals_per_slice(T):
