@@ -297,8 +297,9 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     uint64_t wpol = 0;                                     // L2 policy of this chunk's stores (see SweepParams::res_tasks)
     if (STORE_W) {
         const size_t gband = (size_t)(tile_r0 / RB) + band, tx = tile_c0 / SW_TW;
-        const long long chunk = ((long long)img * ((ny + RB - 1) / RB) + (long long)gband) * p.tiles_x + (long long)tx;
-        wpol = (r0 < ny && chunk * (RB / 2) < p.res_tasks) ? l2_policy_evict_last() : l2_policy_evict_first();
+        // (chosen per CTA, from its first band: uniform, so the policy lives in a uniform register)
+        const long long chunk = ((long long)img * ((ny + RB - 1) / RB) + (long long)(tile_r0 / RB)) * p.tiles_x + (long long)tx;
+        wpol = (chunk * (RB / 2) < p.res_tasks) ? l2_policy_evict_last() : l2_policy_evict_first();
         wchunk = wts + ((((size_t)img * 2 + side) * p.nbands + gband) * p.tiles_x + tx) *
                            (size_t)((2 * a + 1) * (2 * a + 1)) * WSTRIDE;
     }
