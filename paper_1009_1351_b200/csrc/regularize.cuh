@@ -34,7 +34,7 @@
 // Stored weights ("reusing this factor ... instead of recomputing").  The weights
 // belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 the first sweep
 // (STORE_W = true) also writes every unnormalised weight as bf16 into
-// wts[image][side][band][tile_x][delta][RB/2 row pairs][32 lanes][2 rows][4 columns] -- one
+// wts[image][band][tile_x][side][delta][RB/2 row pairs][32 lanes][2 rows][4 columns] -- one
 // contiguous chunk per warp band, written and later read as a sequential stream (DRAM-page
 // friendly; a plane-per-offset layout scatters 256-byte pieces and ran 3x slower); inside a plane
 // the two rows of a pair are interleaved per lane so that the applying sweeps read 16 bytes per
@@ -300,7 +300,7 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
         // (chosen per CTA, from its first band: uniform, so the policy lives in a uniform register)
         const long long chunk = ((long long)img * ((ny + RB - 1) / RB) + (long long)(tile_r0 / RB)) * p.tiles_x + (long long)tx;
         wpol = (chunk * (RB / 2) < p.res_tasks) ? l2_policy_evict_last() : l2_policy_evict_first();
-        wchunk = wts + ((((size_t)img * 2 + side) * p.nbands + gband) * p.tiles_x + tx) *
+        wchunk = wts + ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2 + side) *
                            (size_t)((2 * a + 1) * (2 * a + 1)) * WSTRIDE;
     }
 
@@ -558,8 +558,8 @@ gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
 
     // stage t = (side, dr, k): offsets dr*W + 4k .. of that side's chunk, min(4, W-4k) of them
     const int stages_per_side = W * nchunk, T = 2 * stages_per_side;
-    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)(W * W) * wstride;
-    const __nv_bfloat16 *__restrict__ chunk0 = wts + ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)(W * W) * wstride;
+    const size_t side_stride = (size_t)(W * W) * wstride;       // the two sides of a band are contiguous
+    const __nv_bfloat16 *__restrict__ chunk0 = wts + ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2) * (size_t)(W * W) * wstride;
 
     if (warp == rb) {                               // ---- producer warp: one lane issues the bulk copies
         if (lane == 0) {
@@ -672,7 +672,7 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     const int UW = apply_uw(W), urows = 2 + 2 * a;
     const int rb = p.rb, npairs = rb >> 1;
     const size_t pstride = (size_t)rb * (SW_TW / 8);     // uint4 per offset plane
-    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)WW * pstride;      // uint4
+    const size_t side_stride = (size_t)WW * pstride;     // uint4; the two sides of a band are contiguous
     const size_t npix = (size_t)nx * ny;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
     extern __shared__ float4 smem4[];
@@ -699,7 +699,7 @@ gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
         const int r = gband * rb + 2 * pair, tile_c0 = tx * SW_TW, c0 = tile_c0 + C * lane;
         const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
         const uint4 *__restrict__ wp = reinterpret_cast<const uint4 *>(wts) +
-                                       ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)WW * pstride +
+                                       ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2) * (size_t)WW * pstride +
                                        pair * 32 + lane;
         float nbsum[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
 #pragma unroll 1
@@ -798,6 +798,8 @@ __host__ __device__ inline size_t apply3_smem_bytes(int window, int rb, int dept
     return (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) + (size_t)(rb / 2) * depth * 512;
 }
 
+// (Writing the weight sums Z in the first applying sweep and reading them back in the later ones -- 8 fewer
+// instructions per piece -- was measured here too and left the sweep at 55.7 us: dropped.)
 template <int DEPTH>             // pieces in flight per warp (a power of two)
 __global__ void __launch_bounds__(160, 4)
 gj_apply3_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
@@ -807,7 +809,6 @@ gj_apply3_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
     const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1, WW = W * W;
     const int rb = p.rb, npairs = rb >> 1, urows = rb + 2 * a, UW = apply_uw(W);
     const size_t pstride = (size_t)rb * (SW_TW / 8);     // uint4 per offset plane
-    const size_t side_stride = (size_t)p.nbands * p.tiles_x * (size_t)WW * pstride;      // uint4
     const size_t npix = (size_t)nx * ny;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     extern __shared__ float4 smem4[];
@@ -833,11 +834,10 @@ gj_apply3_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
                          ny, nx, warp, npairs, lane);
     }
     cp_async_commit();
-    // this warp's pieces: 0 .. WW-1 of side 0, then WW .. 2 WW-1 of side 1, one stream
-    const uint4 *__restrict__ ws0 = reinterpret_cast<const uint4 *>(wts) +
-                                    ((((size_t)img * 2) * p.nbands + gband) * p.tiles_x + tx) * (size_t)WW * pstride + warp * 32 + lane;
-    const uint4 *__restrict__ ws1 = ws0 + side_stride;
-    const uint4 *__restrict__ nextp = ws0;
+    // this warp's pieces: 0 .. WW-1 of side 0, then WW .. 2 WW-1 of side 1: one stream at a constant stride (the two
+    // sides of a band are contiguous in the stored layout)
+    const uint4 *__restrict__ nextp = reinterpret_cast<const uint4 *>(wts) +
+                                      ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2) * (size_t)WW * pstride + warp * 32 + lane;
     unsigned issued = 0, wr = ring_s;
     const unsigned total = 2u * (unsigned)WW;
 #pragma unroll 1
@@ -845,49 +845,56 @@ gj_apply3_kernel(SweepParams p, const float *__restrict__ g, const float *__rest
         cp_async16_s_hint(wr, nextp, issued < total, pol);
         cp_async_commit();
         wr += 512;
-        nextp = (issued + 1 == (unsigned)WW) ? ws1 : nextp + pstride;
+        nextp += pstride;
     }
     cp_async_wait<DEPTH - 1>();                               // this thread's window copies have landed
     __syncthreads();                                          // ... and everybody else's
     float nbsum[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-    unsigned t = 0;
+    unsigned rd = 0;                                          // ring offset of the piece consumed next
+    const int wfull = W & ~3, wtail = W & 3;                  // offsets of a window row in groups of four, and the rest
 #pragma unroll 1
     for (int sd = 0; sd < 2; ++sd) {
         float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
         const float *__restrict__ uwin = sU + (sd * urows + 2 * warp) * UW + C * lane;
+        // one piece: issue the piece DEPTH-1 ahead, wait for the oldest, accumulate its 2 x 4 weights
+        auto piece = [&](const float (&uw0)[8], const float (&uw1)[8], int jj) {
+            cp_async16_s_hint(wr, nextp, issued < total, pol);
+            cp_async_commit();                                // (empty groups keep the wait count uniform)
+            ++issued;
+            nextp += pstride;
+            wr = (wr == ring_s + (DEPTH - 1) * 512) ? ring_s : wr + 512;
+            cp_async_wait<DEPTH - 1>();                       // the oldest piece has landed (this lane's own 16 bytes)
+            const uint4 wv = lds128_s(ring_s + rd);
+            rd = (rd + 512) & ((DEPTH - 1) << 9);
+            // bf16 -> fp32 is a 16-bit shift: low half << 16, high half masked
+            const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
+                                 __uint_as_float(wv.y << 16), __uint_as_float(wv.y & 0xffff0000u)};
+            const float w1[C] = {__uint_as_float(wv.z << 16), __uint_as_float(wv.z & 0xffff0000u),
+                                 __uint_as_float(wv.w << 16), __uint_as_float(wv.w & 0xffff0000u)};
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                Z[0][c] += w0[c];
+                A[0][c] = fmaf(w0[c], uw0[c + jj], A[0][c]);
+                Z[1][c] += w1[c];
+                A[1][c] = fmaf(w1[c], uw1[c + jj], A[1][c]);
+            }
+        };
 #pragma unroll 1
         for (int dr = 0; dr < W; ++dr) {
             const float *__restrict__ urow0 = uwin + dr * UW;
 #pragma unroll 1
-            for (int k = 0; k < W; k += 4) {
+            for (int k = 0; k <= W - 1; k += 4) {
                 const float4 ua = *reinterpret_cast<const float4 *>(urow0 + k), ub = *reinterpret_cast<const float4 *>(urow0 + k + 4);
                 const float4 uc = *reinterpret_cast<const float4 *>(urow0 + UW + k), ud = *reinterpret_cast<const float4 *>(urow0 + UW + k + 4);
                 const float uw0[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
                 const float uw1[8] = {uc.x, uc.y, uc.z, uc.w, ud.x, ud.y, ud.z, ud.w};
-                const int noff = min(4, W - k);
+                if (k < wfull) {                              // a full group of four offsets: no per-piece test
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    if (jj < noff) {
-                        cp_async16_s_hint(wr, nextp, issued < total, pol);
-                        cp_async_commit();                    // (empty groups keep the wait count uniform)
-                        ++issued;
-                        nextp = (issued == (unsigned)WW) ? ws1 : nextp + pstride;
-                        wr = (wr == ring_s + (DEPTH - 1) * 512) ? ring_s : wr + 512;
-                        cp_async_wait<DEPTH - 1>();           // piece t has landed (this lane's own 16 bytes)
-                        const uint4 wv = lds128_s(ring_s + ((t & (DEPTH - 1)) << 9));
-                        ++t;
-                        const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
-                                             __uint_as_float(wv.y << 16), __uint_as_float(wv.y & 0xffff0000u)};
-                        const float w1[C] = {__uint_as_float(wv.z << 16), __uint_as_float(wv.z & 0xffff0000u),
-                                             __uint_as_float(wv.w << 16), __uint_as_float(wv.w & 0xffff0000u)};
+                    for (int jj = 0; jj < 4; ++jj) piece(uw0, uw1, jj);
+                } else {
 #pragma unroll
-                        for (int c = 0; c < C; ++c) {
-                            Z[0][c] += w0[c];
-                            A[0][c] = fmaf(w0[c], uw0[c + jj], A[0][c]);
-                            Z[1][c] += w1[c];
-                            A[1][c] = fmaf(w1[c], uw1[c + jj], A[1][c]);
-                        }
-                    }
+                    for (int jj = 0; jj < 3; ++jj)
+                        if (jj < wtail) piece(uw0, uw1, jj);
                 }
             }
         }

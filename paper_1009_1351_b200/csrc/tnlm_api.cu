@@ -72,7 +72,7 @@ struct tnlm_handle {
     float *d_imI = nullptr;                                                  // its interleaved copy (groups of four slices)
     float *d_r = nullptr, *d_rw = nullptr, *d_q = nullptr, *d_sw = nullptr;  // sinograms (d_sw = sqrt(w))
     float *d_yh = nullptr, *d_wh = nullptr;                                  // host-API staging
-    __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps, [S*N][2][W*W][ny][nx]
+    __nv_bfloat16 *d_wts = nullptr;          // stored weights of the sweeps (layout: regularize.cuh)
     size_t wts_cap = 0;               // in halves
     size_t apply_smem = 0;
     double *d_scal = nullptr;
@@ -937,12 +937,7 @@ static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_s
     const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
     if (H->opt_cache_mb <= 0 || need * sizeof(__nv_bfloat16) > (size_t)H->opt_cache_mb * 1048576ull) return nullptr;
     if (need > H->wts_cap) {
-        if (H->d_wts) {
-        cudaFree(H->d_wts);
-        // the evict_last lines of the stored weights (apply_resident_mb) would otherwise keep their L2 priority
-        // until something else claims it; ignore a driver that does not support the call
-        if (cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
-    }
+        if (H->d_wts) cudaFree(H->d_wts);
         H->d_wts = nullptr; H->wts_cap = 0;
         if (cudaMalloc(&H->d_wts, need * sizeof(__nv_bfloat16)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
         H->wts_cap = need;
