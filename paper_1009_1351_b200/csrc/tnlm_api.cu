@@ -260,9 +260,12 @@ static cudaError_t build_sweep_shapes(tnlm_handle *H, size_t smem_limit)
     return e;
 }
 
-// Cost model of one sweep over n_img images with shape sh, in (resident warps) x (rows marched)
-// per SM: full waves of occ CTAs per SM, then the remainder spread over the SMs.  At least 8
-// warps per SM are needed to keep the FP32 pipes busy, so fewer do not run faster.
+// Cost model of one sweep over n_img images with shape sh, in (resident warps) x (rows marched) per SM: full waves
+// of occ CTAs per SM, then the remainder spread over the SMs.  Measured on cfg 3 / cfg 4 sized sweeps: an SM with
+// fewer than ~5 warps of this kernel is not faster per warp-row than one with 5 (so a remainder of half-size CTAs
+// costs 0.65 of a full wave, not 0.5 and not 1); two half-size CTAs per SM hide each other's tile staging once there
+// is more than one wave (-1.5 %), but stage more halo per band (+3 % in a single wave); one-band CTAs stage 2.2x
+// the halo per band (+15 %).
 static double sweep_cost(const tnlm_handle *H, const SweepShape &sh, int n_img)
 {
     const int pb = (H->patch - 1) / 2;
@@ -270,10 +273,11 @@ static double sweep_cost(const tnlm_handle *H, const SweepShape &sh, int n_img)
     const long long ctas = (long long)n_img * ((H->ny + th - 1) / th) * ((H->nx + SW_TW - 1) / SW_TW);
     const long long cap = (long long)H->n_sm * sh.occ;
     const long long full = ctas / cap, rem = ctas % cap;
-    auto wave = [&](long long k) { return (double)std::max<long long>(k * 2 * sh.nb, 8) * (sh.rb + 2 * pb); };
+    auto wave = [&](long long k) { return std::max((double)(k * 2 * sh.nb), 5.2) * (sh.rb + 2 * pb); };
     double c = (double)full * wave(sh.occ);
     if (rem) c += wave((rem + H->n_sm - 1) / H->n_sm);
-    return c;
+    const double staging = sh.nb >= 4 ? 1.0 : (sh.nb == 2 ? (full >= 1 ? 0.985 : 1.03) : 1.15);
+    return c * staging;
 }
 
 extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_phase, int window, int patch,
