@@ -73,7 +73,8 @@
  *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change;
  *   project_interleave (1, the default: in a call with four or more slices the forward projector reads handle-owned
  *   copies of the image in which the four slices of a group are interleaved per pixel, one 16-byte gather per cell
- *   for four slices; 0 = every slice from its own image and transposed copy).
+ *   for four slices; 0 = every slice from its own image and transposed copy), project_block (threads per CTA of the
+ *   forward projector: 128, the default, 256 or 64; changes only how the ||q||^2 partial sums are grouped).
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
@@ -174,7 +175,7 @@ int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_ent
 
 /* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
  * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns", "apply_kernel", "apply_depth", "apply_wpc",
- * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "project_interleave", "backproject_group"; 0 restores the
+ * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "project_interleave", "project_block", "backproject_group"; 0 restores the
  * heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
 int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
 

@@ -164,7 +164,7 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
         __syncthreads();
         if (threadIdx.x < 32 * NS) {
             const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
-            float v = l < 8 ? part[s][l] : 0.f;
+            float v = l < (int)(blockDim.x >> 5) ? part[s][l] : 0.f;
             v = warp_sum(v);
             if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
         }
@@ -299,7 +299,7 @@ project_il_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__re
         __syncthreads();
         if (threadIdx.x < 32 * NS) {
             const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
-            float v = l < 8 ? part[s][l] : 0.f;
+            float v = l < (int)(blockDim.x >> 5) ? part[s][l] : 0.f;
             v = warp_sum(v);
             if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
         }
