@@ -80,11 +80,11 @@ def projector_work(cfg, n_slices):
     forward ~10 flop per ray segment, 1.3 L segments per ray; gather backprojection ~76 flop per
     pixel-view; bytes = image + sinogram once (4 L^2 + 4 V B per phase).  The slices of a batch share the
     geometry, so the library evaluates the ray walk (6 of the 10 flops of a segment) once per group of 4 slices
-    and the candidate geometry (66 of the 76 flops of a pixel-view) once per group of 8: the *_shared counts are
+    and the candidate geometry (66 of the 76 flops of a pixel-view) once per group of 16: the *_shared counts are
     the flops that formulation needs, reported beside the per-slice counts so that no fraction is padded."""
     n = n_slices * cfg.N
     gf = 4 if n_slices >= 4 else 1          # slices per forward group (project_il_kernel)
-    gb = 8 if n_slices >= 8 else (4 if n_slices >= 4 else (2 if n_slices >= 2 else 1))
+    gb = 16 if n_slices >= 16 else (8 if n_slices >= 8 else (4 if n_slices >= 4 else (2 if n_slices >= 2 else 1)))
     return {"project_flops": n * cfg.V * cfg.B * 1.3 * cfg.L * 10.0,
             "project_flops_shared": n * cfg.V * cfg.B * 1.3 * cfg.L * (6.0 / gf + 4.0),
             "backproject_flops": n * cfg.L * cfg.L * cfg.V * 76.0,

@@ -68,7 +68,7 @@
  *   apply_snake (1, the default: successive stored-weight sweeps deal their tasks in opposite orders, so a sweep
  *   starts on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored
  *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first),
- *   backproject_group (8, the default; 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
+ *   backproject_group (16, the default; 8, 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
  *   share the geometry (nothing couples them, L77), so one thread of a projector serves up to that many slices
  *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change;
  *   project_interleave (1, the default: in a call with four or more slices the forward projector reads handle-owned

@@ -1,6 +1,6 @@
 // projector.cuh -- fan-beam forward projector P (ray-driven, one thread per (view,bin)) and its
 // matched adjoint P^T (pixel-driven gather, one thread per 2 x 2 pixel block).  PAPER.md:L75, L79, L212.
-// The slices of a batch share the ray geometry: up to 8 slices per thread in the adjoint, groups of 4 slices
+// The slices of a batch share the ray geometry: up to 16 slices per thread in the adjoint, groups of 4 slices
 // interleaved per pixel in the forward projector (project_il_kernel).
 // Both kernels evaluate tnlm::ray_cum on the same RayEntry table, so every matrix entry
 // len(ray ∩ pixel) is bit-identical on the two sides and P^T is the exact transpose of P (common.cuh).

@@ -53,7 +53,7 @@ struct tnlm_handle {
     int opt_project_il = 1;         // forward projector: groups of four slices read interleaved copies (project_il_kernel)
     int opt_project_block = 128;    // project_kernel / project_il_kernel: threads per CTA (256, 128, 64; 128 measured 2-3 % faster than 256: tail balance)
     int opt_project_group = 1;      // project_kernel: at most this many slices of a batch per thread (4, 2 or 1)
-    int opt_backproject_group = 8;  // backproject_kernel: the same (8, 4, 2 or 1)
+    int opt_backproject_group = 16; // backproject_kernel: the same (16, 8, 4, 2 or 1)
     int opt_snake = 1;      // gj_apply2_kernel: successive sweeps deal their tasks in opposite orders
     long long opt_resident_mb = 32;   // MB of stored weights marked evict_last in L2 (the rest evict_first); 0 = none
     // geometry tables (device)
@@ -614,12 +614,13 @@ static int launch_backproject_groups(tnlm_handle *H, const float *sino, float *i
 {
     const int max_ns = H->opt_backproject_group;
     int s0 = 0;
-    for (int ns = 8; ns >= 1; ns >>= 1) {
+    for (int ns = 16; ns >= 1; ns >>= 1) {
         if (ns > max_ns) continue;
         const int groups = (n_slices - s0) / ns;
         if (groups < 1) continue;
         dim3 grid((H->nx + 8 * BC - 1) / (8 * BC), (H->ny + 16 * BR - 1) / (16 * BR), groups * H->n_phase);
-        if (ns == 8) backproject_kernel<POLY, 8, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        if (ns == 16) backproject_kernel<POLY, 16, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
+        else if (ns == 8) backproject_kernel<POLY, 8, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
         else if (ns == 4) backproject_kernel<POLY, 4, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
         else if (ns == 2) backproject_kernel<POLY, 2, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
         else backproject_kernel<POLY, 1, BR, BC><<<grid, 128, 0, st>>>(H->G, H->d_tab, H->d_views, H->d_split, sino, img, red, s0);
@@ -1029,7 +1030,7 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "project_interleave") { if ((ok = in(0, 1))) H->opt_project_il = (int)value; }
     else if (n == "project_block") { if ((ok = (value == 256 || value == 128 || value == 64))) H->opt_project_block = (int)value; }
     else if (n == "project_group") { if ((ok = (value == 1 || value == 2 || value == 4))) H->opt_project_group = (int)value; }
-    else if (n == "backproject_group") { if ((ok = (value == 1 || value == 2 || value == 4 || value == 8))) H->opt_backproject_group = (int)value; }
+    else if (n == "backproject_group") { if ((ok = (value == 1 || value == 2 || value == 4 || value == 8 || value == 16))) H->opt_backproject_group = (int)value; }
     else if (n == "apply_snake") { if ((ok = in(0, 1))) H->opt_snake = (int)value; }
     else if (n == "apply_resident_mb") { if ((ok = in(0, 1 << 20))) H->opt_resident_mb = value; }
     else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);

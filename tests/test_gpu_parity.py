@@ -184,20 +184,21 @@ def test_strip_and_gather_forward_projectors_are_bit_identical(T, cfg):
 
 def test_slice_groups_share_geometry_bit_identically(T):
     # Slices of a batch have one geometry: the projectors serve groups of 8/4/2/1 slices per thread
-    # (options backproject_group, project_group).  S = 11 = 8 + 2 + 1 exercises every group size and the
-    # remainders; per slice the arithmetic is that of a single slice: bit-identical, and equal to the oracle.
+    # (options backproject_group, project_group).  S = 23 = 16 + 4 + 2 + 1 (= 8 + 8 + 4 + 2 + 1 ...) exercises every
+    # group size and the remainders; per slice the arithmetic is that of a single slice: bit-identical, and equal
+    # to the oracle.
     torch, tn = T
     cfg = small_geom_cfg(L=37, N=2, V=23, B=61)
     hd, og = handles(tn, cfg)
-    S = 11
+    S = 23
     rng = np.random.default_rng(5)
     img = rng.random((S, cfg.N, cfg.L, cfg.L)) * 0.02
     sino = rng.random((S, cfg.N, cfg.V, cfg.B))
     w = rng.random((S, cfg.N, cfg.V, cfg.B)) * 50 + 1
     imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
     ref = {}
-    # project_interleave: slices 0..7 through the interleaved copies (project_il_kernel, cgls_update_us_il), 8..10 not
-    for pg, bg, il in [(1, 1, 0), (2, 2, 0), (4, 4, 0), (4, 8, 1), (1, 8, 1), (2, 1, 1)]:
+    # project_interleave: slices 0..19 through the interleaved copies (project_il_kernel, cgls_update_us_il), 20..22 not
+    for pg, bg, il in [(1, 1, 0), (2, 2, 0), (4, 4, 0), (4, 8, 1), (1, 16, 1), (2, 1, 1), (1, 16, 0)]:
         tn.set_option(hd, "project_kernel", 0); tn.set_option(hd, "project_group", pg); tn.set_option(hd, "backproject_group", bg)
         tn.set_option(hd, "project_interleave", il)
         po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
@@ -205,7 +206,7 @@ def test_slice_groups_share_geometry_bit_identically(T):
         tn.cgls_step(hd, imgd, sinod, wd, 3, go)          # fused epilogues and per-problem reductions of every slice
         if not ref:
             ref = dict(p=po, b=bo, g=go)
-            for s in (0, 7, 8, 10):
+            for s in (0, 15, 16, 22):
                 assert rel(po[s].cpu().numpy(), oracle.project(og, img[s])) < 2e-6
                 assert rel(bo[s].cpu().numpy(), oracle.backproject(og, sino[s], cfg.L, cfg.L)) < 2e-6
                 assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 3)) < STEP_TOL
