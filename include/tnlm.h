@@ -167,6 +167,40 @@ int tnlm_reconstruct_host(tnlm_handle *handle, const float *y_host, const float 
 /* Message of the last failing call on this handle ("" if none); handle-owned, valid until the
  * next call on the handle.  NULL handle -> message of the calling thread's last failed tnlm_create. */
 const char *tnlm_last_error(const tnlm_handle *handle);
+/* tnlm_regularize_step for callers that must not allocate device memory.
+ *
+ * Who that is: a reconstruction service whose HBM is already handed out in full (to a framework's
+ * caching allocator holding a 64-slice batch, or to another job sharing the GPU), where cudaMalloc
+ * fails; and a scanner-side loop that keeps other streams busy (the upload of the next slice, a display
+ * kernel) and cannot take the device-wide synchronisation cudaMalloc implies.  tnlm_regularize_step
+ * allocates its ping-pong images and stored weights on first use, so neither can call it unprepared.
+ *
+ * What it does: the same result as tnlm_regularize_step (weights of g, m2 Gauss-Jacobi sweeps, clip;
+ * same arguments, f_out may alias g), with the weights recomputed in fp32 in every sweep (nothing is
+ * stored) and the intermediate sweeps written to a scratch array that is compiled into the library
+ * (a file-scope __device__ array of 2 * TNLM_NOALLOC_MAX_PIXELS floats = 20 MiB).  It calls no
+ * cudaMalloc, cudaFree or any other allocating routine; a TNLM-only handle (geometry = NULL) owns no
+ * device memory either, so with such a handle the whole path is allocation-free.  Per-launch timing
+ * (tnlm_profile_kernels) does not cover this call, because recording would create events.
+ *
+ * Limits and sharp edges
+ *   - n_slices * n_phase * ny * nx must not exceed TNLM_NOALLOC_MAX_PIXELS (one 10-phase 512 x 512
+ *     slice); larger calls return TNLM_UNSUPPORTED with a message naming both numbers.
+ *   - The array is part of the library's device image: every GPU on which the library's CUDA code is
+ *     loaded holds those 20 MiB until the process exits, whether or not this call is ever made.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with
+ *     that device current), which can make the CUDA runtime load the library's device code.  Make
+ *     that first call during set-up, before any stream capture is begun.
+ *   - There is ONE array per device, shared by every handle, stream and thread.  Two calls that
+ *     overlap on the GPU (different streams, or different handles without ordering between them) race on
+ *     it and corrupt each other's sweeps; order them on one stream or with events.
+ *   - The array keeps what the last call left in it.  Nothing has to be cleared: every sweep writes
+ *     every pixel of its destination before the next sweep reads it, and pixels beyond the current
+ *     call's size are never read. */
+#define TNLM_NOALLOC_MAX_PIXELS 2621440
+int tnlm_regularize_step_noalloc(tnlm_handle *handle, const float *g, int m2, float *f_out,
+                                 int n_slices, void *stream);
+
 
 /* Allocate now everything a later tnlm_cgls_step / tnlm_regularize_step / tnlm_reconstruct call
  * with up to n_slices slices, m1 CGLS steps and m2 sweeps would allocate on first use

@@ -9,4 +9,4 @@ fallback: if the library is missing or no CUDA device is present the calls fail 
 from .binding import (Geometry, Handle, TnlmError, cgls_step, create, lib_path, library,  # noqa: F401
                       backproject, project, reconstruct, regularize_step, reconstruct_host,
                       regularize_step_host, version, profile_kernels, kernel_times, fbp_init, fma_peak,
-                      reserve, set_option)
+                      reserve, set_option, regularize_step_noalloc, NOALLOC_MAX_PIXELS)

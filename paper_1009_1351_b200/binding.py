@@ -15,7 +15,10 @@ EXPORTS = ["tnlm_create", "tnlm_destroy", "tnlm_project", "tnlm_backproject", "t
            "tnlm_regularize_step", "tnlm_reconstruct", "tnlm_regularize_step_host",
            "tnlm_reconstruct_host", "tnlm_last_error", "tnlm_launch_count", "tnlm_version",
            "tnlm_profile_kernels", "tnlm_kernel_times", "tnlm_fbp_init", "tnlm_fma_peak",
-           "tnlm_reserve", "tnlm_set_option", "tnlm_device"]
+           "tnlm_reserve", "tnlm_set_option", "tnlm_device", "tnlm_regularize_step_noalloc"]
+
+# TNLM_NOALLOC_MAX_PIXELS of include/tnlm.h: the most pixels (n_slices * n_phase * ny * nx) regularize_step_noalloc takes
+NOALLOC_MAX_PIXELS = 2621440
 
 # tnlm_kernel_kind
 KERNEL_KINDS = {0: "sweep", 1: "sweep_store", 2: "apply", 3: "project", 4: "backproject", 5: "transpose",
@@ -69,6 +72,7 @@ def library():
         L.tnlm_backproject.argtypes = [P, P, P, I, P]
         L.tnlm_cgls_step.argtypes = [P, P, P, P, I, P, I, P]
         L.tnlm_regularize_step.argtypes = [P, P, I, P, I, P]
+        L.tnlm_regularize_step_noalloc.argtypes = [P, P, I, P, I, P]
         L.tnlm_reconstruct.argtypes = [P, P, P, P, I, I, I, P, I, P]
         L.tnlm_regularize_step_host.argtypes = [P, P, I, P, I, P]
         L.tnlm_reconstruct_host.argtypes = [P, P, P, P, I, I, I, P, I, P]
@@ -204,6 +208,22 @@ def regularize_step(h: Handle, g, m2, f_out, stream=None):
     S = _slices(g, h.img_per_slice, "g")
     h.check(library().tnlm_regularize_step(h.ptr, _dev(h, g, "g"), m2, _dev(h, f_out, "f_out", S * h.img_per_slice), S,
                                            _stream(stream)))
+    return f_out
+
+
+def regularize_step_noalloc(h: Handle, g, m2, f_out, stream=None):
+    """tnlm_regularize_step_noalloc: regularize_step for callers that must not allocate device memory.
+
+    Use it when cudaMalloc is off the table: all of HBM already belongs to another allocator (torch's caching
+    allocator holding a large batch, say), or other streams are busy and must not be stalled by the device-wide
+    synchronisation an allocation implies.  The sweeps ping-pong through a 20 MiB array compiled into the
+    library instead of handle-owned buffers, and the weights are recomputed in fp32 in every sweep.  At most
+    NOALLOC_MAX_PIXELS pixels per call (larger raises TnlmError, TNLM_UNSUPPORTED); the array is shared by every
+    handle and stream of a device, so calls that overlap on the GPU race; make the first call on a device during
+    set-up (it looks up the array's address), before any stream capture."""
+    S = _slices(g, h.img_per_slice, "g")
+    h.check(library().tnlm_regularize_step_noalloc(h.ptr, _dev(h, g, "g"), m2,
+                                                   _dev(h, f_out, "f_out", S * h.img_per_slice), S, _stream(stream)))
     return f_out
 
 

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1118,6 +1119,72 @@ extern "C" int tnlm_reconstruct(tnlm_handle *H, const float *y, const float *w, 
     ENTER(H, "tnlm_reconstruct", n_slices, true);
     int rc;
     if (!y || !f_out) return fail(H, TNLM_INVALID_ARG, "y and f_out must not be NULL");
+// ------------------------------------------------------------------------------ TNLM step without allocation
+// tnlm_regularize_step_noalloc (tnlm.h): for callers that cannot cudaMalloc -- HBM fully handed out to someone
+// else's allocator, or other streams that must not be stalled by cudaMalloc's device-wide synchronisation.
+// The two ping-pong images of the sweeps live in this array instead of the handle's cudaMalloc'ed d_ua / d_ub.
+// It is part of the device image of this translation unit: 20 MiB on every GPU that loads it, until exit.
+// One array per device, shared by all handles and streams: overlapping calls race (documented in tnlm.h).
+static __device__ __align__(256) float g_noalloc_scratch[2 * (size_t)TNLM_NOALLOC_MAX_PIXELS];
+
+// Device address of g_noalloc_scratch on the CURRENT device.  In host code the name g_noalloc_scratch is only a
+// stand-in the runtime keys its lookup on, not a pointer a kernel may be given; the address differs per device, so
+// it is looked up once per device, with that device current, and remembered.
+static cudaError_t noalloc_scratch_address(int device, float **out)
+{
+    static std::mutex lock;
+    static float *known[64] = {};
+    std::lock_guard<std::mutex> hold(lock);
+    if (device >= 0 && device < 64 && known[device]) { *out = known[device]; return cudaSuccess; }
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if (device >= 0 && device < 64) known[device] = static_cast<float *>(p);
+    *out = static_cast<float *>(p);
+    return cudaSuccess;
+}
+
+extern "C" int tnlm_regularize_step_noalloc(tnlm_handle *H, const float *g, int m2, float *f_out, int n_slices, void *stream)
+{
+    ENTER(H, "tnlm_regularize_step_noalloc", n_slices, false);      // makes H->device current
+    int rc;
+    if (!g || !f_out) return fail(H, TNLM_INVALID_ARG, "g and f_out must not be NULL");
+    if (m2 < 0) return fail(H, TNLM_INVALID_ARG, "m2 must be >= 0");
+    const size_t n = (size_t)n_slices * H->n_phase * H->nx * H->ny;
+    if (n > (size_t)TNLM_NOALLOC_MAX_PIXELS)
+        return fail(H, TNLM_UNSUPPORTED, "tnlm_regularize_step_noalloc: n_slices * n_phase * ny * nx = " + std::to_string(n) +
+                    " pixels is above the built-in scratch of TNLM_NOALLOC_MAX_PIXELS = " + std::to_string(TNLM_NOALLOC_MAX_PIXELS) +
+                    "; use tnlm_regularize_step (which allocates) or fewer slices per call");
+    float *scratch = nullptr;
+    CU(H, noalloc_scratch_address(H->device, &scratch));
+    cudaStream_t st = (cudaStream_t)stream;
+    // per-launch timing would create events (prof_mark): not in a call that promises to allocate nothing
+    struct ProfOff {
+        tnlm_handle *H; bool was;
+        explicit ProfOff(tnlm_handle *h) : H(h), was(h->prof) { h->prof = false; }
+        ~ProfOff() { H->prof = was; }
+    } prof_off(H);
+    if (m2 == 0) {
+        clip_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g, f_out, n);
+        LAUNCHED(H);
+        return TNLM_OK;
+    }
+    const bool alias = (f_out == g);
+    const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
+    if (!sh) return TNLM_INVALID_ARG;
+    float *pp[2] = {scratch, scratch + TNLM_NOALLOC_MAX_PIXELS};
+    const float *src = g;
+    for (int m = 0; m < m2; ++m) {
+        const bool last = (m + 1 == m2);
+        float *dst = (last && !alias) ? f_out : pp[m & 1];   // every sweep writes all n pixels of dst: no clearing needed
+        if ((rc = launch_sweep(H, *sh, g, src, dst, last ? 1 : 0, n_slices, nullptr, st))) return rc;   // weights of g, fp32, every sweep
+        src = dst;
+    }
+    if (alias) CU(H, cudaMemcpyAsync(f_out, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return TNLM_OK;
+}
+
     if (k_outer < 0 || m1 < 0 || m2 < 0) return fail(H, TNLM_INVALID_ARG, "k_outer, m1, m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
     return reconstruct_device(H, y, w, f0, k_outer, m1, m2, f_out, n_slices, (cudaStream_t)stream);
