@@ -40,10 +40,10 @@
  *   Device entry points enqueue work on `stream` (a cudaStream_t passed as void*, NULL = the
  *   legacy default stream) and return without waiting for it; all scalars of CGLS stay on the
  *   device.  The FIRST call that needs a workspace buffer of some kind, and any call with a larger
- *   n_slices than seen before, allocates it with cudaMalloc inside the call, which synchronises
- *   the device; tnlm_reserve does all of that up front, after which the enqueue calls never
- *   allocate.  `_host` entry points copy in, run, copy out and synchronise `stream` before
- *   returning.  A handle belongs to the CUDA device that was current at tnlm_create: every entry
+ *   n_slices than seen before, allocates it with cudaMalloc inside the call (a larger n_slices first
+ *   releases every workspace buffer of the handle with cudaFree); both synchronise the device.
+ *   tnlm_reserve does all of that up front, after which the enqueue calls never allocate or free.
+ *   `_host` entry points copy in, run, copy out and synchronise `stream` before returning.  A handle belongs to the CUDA device that was current at tnlm_create: every entry
  *   point makes that device current for the call and restores the caller's; device pointers and
  *   the stream must belong to it.  A handle must not be used from two streams or threads at once.
  *
@@ -67,7 +67,9 @@
  *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers),
  *   apply_snake (1, the default: successive stored-weight sweeps deal their tasks in opposite orders, so a sweep
  *   starts on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored
- *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first),
+ *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first;
+ *   tnlm_destroy does not reset the context's persisting L2 lines -- that would hit every other user of the
+ *   context -- so those lines keep their priority until other evict_last traffic displaces them),
  *   backproject_group (16, the default; 8, 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
  *   share the geometry (nothing couples them, L77), so one thread of a projector serves up to that many slices
  *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change;
@@ -78,7 +80,8 @@
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
- *   finite for |u| < 2^17 (1.3e5; HU-scaled images are fine).  h must be <= 1e12.
+ *   finite for |u| < 2^17 (1.3e5; HU-scaled images are fine).  h must be <= 1e12, and large enough for
+ *   log2(e)/h^2 to be a finite fp32 number (h > 7e-20); tnlm_create refuses others.
  *
  * Errors
  *   Every call returns a tnlm_status; nothing throws, exits or falls back to the CPU.
@@ -164,9 +167,6 @@ int tnlm_reconstruct_host(tnlm_handle *handle, const float *y_host, const float 
                           const float *f0_host, int k_outer, int m1, int m2, float *f_out_host,
                           int n_slices, void *stream);
 
-/* Message of the last failing call on this handle ("" if none); handle-owned, valid until the
- * next call on the handle.  NULL handle -> message of the calling thread's last failed tnlm_create. */
-const char *tnlm_last_error(const tnlm_handle *handle);
 /* tnlm_regularize_step for callers that must not allocate device memory.
  *
  * Who that is: a reconstruction service whose HBM is already handed out in full (to a framework's
@@ -201,6 +201,9 @@ const char *tnlm_last_error(const tnlm_handle *handle);
 int tnlm_regularize_step_noalloc(tnlm_handle *handle, const float *g, int m2, float *f_out,
                                  int n_slices, void *stream);
 
+/* Message of the last failing call on this handle ("" if none); handle-owned, valid until the
+ * next call on the handle.  NULL handle -> message of the calling thread's last failed tnlm_create. */
+const char *tnlm_last_error(const tnlm_handle *handle);
 
 /* Allocate now everything a later tnlm_cgls_step / tnlm_regularize_step / tnlm_reconstruct call
  * with up to n_slices slices, m1 CGLS steps and m2 sweeps would allocate on first use

@@ -242,7 +242,9 @@ def reserve(h: Handle, n_slices, m1, m2, host_entry_points=False):
 
 
 def set_option(h: Handle, name: str, value: int):
-    """tnlm_set_option: "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns"."""
+    """tnlm_set_option: a tuning option of this handle; the names and ranges are those of include/tnlm.h
+    ("Stored weights and tuning knobs"), e.g. "weight_cache_mb" (0 = recompute the weights in fp32 every sweep).
+    Unknown names and out-of-range values raise TnlmError (TNLM_INVALID_ARG)."""
     h.check(library().tnlm_set_option(h.ptr, name.encode(), int(value)))
 
 

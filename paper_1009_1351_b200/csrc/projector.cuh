@@ -162,9 +162,10 @@ project_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__restr
             if ((threadIdx.x & 31) == 0) part[s][threadIdx.x >> 5] = v;
         }
         __syncthreads();
-        if (threadIdx.x < 32 * NS) {
-            const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
-            float v = l < (int)(blockDim.x >> 5) ? part[s][l] : 0.f;
+        // warp w sums slices w, w + warps, ...: a CTA of 64 threads (project_block = 64) has fewer warps than NS = 4 slices
+        const int nwarp = (int)(blockDim.x >> 5), l = threadIdx.x & 31;
+        for (int s = threadIdx.x >> 5; s < NS; s += nwarp) {
+            float v = l < nwarp ? part[s][l] : 0.f;
             v = warp_sum(v);
             if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
         }
@@ -297,9 +298,10 @@ project_il_kernel(Geom G, const RayEntry *__restrict__ tab, const RayRange *__re
             if ((threadIdx.x & 31) == 0) part[s][threadIdx.x >> 5] = v;
         }
         __syncthreads();
-        if (threadIdx.x < 32 * NS) {
-            const int s = threadIdx.x >> 5, l = threadIdx.x & 31;
-            float v = l < (int)(blockDim.x >> 5) ? part[s][l] : 0.f;
+        // warp w sums slices w, w + warps, ...: a CTA of 64 threads (project_block = 64) has fewer warps than NS = 4 slices
+        const int nwarp = (int)(blockDim.x >> 5), l = threadIdx.x & 31;
+        for (int s = threadIdx.x >> 5; s < NS; s += nwarp) {
+            float v = l < nwarp ? part[s][l] : 0.f;
             v = warp_sum(v);
             if (l == 0) atomicAdd(red + prob + s * G.n_phase, (double)v);
         }

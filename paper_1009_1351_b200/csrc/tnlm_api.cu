@@ -80,7 +80,7 @@ struct tnlm_handle {
     double *d_scal = nullptr;
     int scal_cap = 0;
     long long launches = 0;
-    // optional per-launch timing of the TNLM kernels (tnlm_profile_sweeps)
+    // optional per-launch timing of every kernel of the path (tnlm_profile_kernels / tnlm_kernel_times)
     bool prof = false;
     std::vector<cudaEvent_t> prof_ev;     // 2 events per timed launch
     std::vector<int> prof_kind;
@@ -282,6 +282,14 @@ static double sweep_cost(const tnlm_handle *H, const SweepShape &sh, int n_img)
     return c * staging;
 }
 
+// Does some launchable sweep shape have rb rows per band and nb bands per CTA (0 = any)?
+static bool sweep_shape_known(const tnlm_handle *H, int rb, int nb)
+{
+    for (const SweepShape &sh : H->shapes)
+        if ((!rb || sh.rb == rb) && (!nb || sh.nb == nb)) return true;
+    return false;
+}
+
 extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_phase, int window, int patch,
                            float h, float mu, tnlm_handle **out)
 {
@@ -293,6 +301,8 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
         return fail(nullptr, TNLM_INVALID_ARG, "window and patch must be odd and >= 1");
     if (!(h > 0.f) || !std::isfinite(h)) return fail(nullptr, TNLM_INVALID_ARG, "h must be finite and > 0");
     if (h > 1e12f) return fail(nullptr, TNLM_INVALID_ARG, "h above 1e12: excluded candidates could no longer be given weight 0");
+    if (!std::isfinite((float)(1.4426950408889634 / ((double)h * (double)h))))
+        return fail(nullptr, TNLM_INVALID_ARG, "h below 1e-19: log2(e)/h^2 overflows fp32 (a zero patch distance would give NaN)");
     if (!(mu >= 0.f) || !std::isfinite(mu)) return fail(nullptr, TNLM_INVALID_ARG, "mu must be finite and >= 0");
     if (patch > MAX_PATCH || window > MAX_WINDOW)
         return fail(nullptr, TNLM_UNSUPPORTED, "patch > 9 or window > 31 not compiled");
@@ -321,7 +331,12 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     H->device = dev;
     if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) H->opt_cache_mb = std::strtoll(ev, nullptr, 10);
     if (const char *ev = std::getenv("TNLM_SWEEP_SHAPE")) std::sscanf(ev, "%d,%d", &H->opt_rb, &H->opt_nb);
-    if (const char *ev = std::getenv("TNLM_APPLY_NS")) H->opt_ns = std::atoi(ev);
+    if (const char *ev = std::getenv("TNLM_APPLY_NS")) {
+        char *end = nullptr;
+        const long v = std::strtol(ev, &end, 10);
+        if (end == ev || *end || v < 0 || v > AP_NS_MAX) { delete H; return fail(nullptr, TNLM_INVALID_ARG, "TNLM_APPLY_NS must be an integer in [0, " + std::to_string(AP_NS_MAX) + "]"); }
+        H->opt_ns = (int)v;
+    }
 
     // TNLM parameters
     SweepParams &R = H->R;
@@ -357,6 +372,10 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     if (H->shapes.empty()) {
         delete H;
         return fail(nullptr, TNLM_UNSUPPORTED, "window/patch need more shared memory than one CTA has");
+    }
+    if (!sweep_shape_known(H, H->opt_rb, H->opt_nb)) {
+        delete H;
+        return fail(nullptr, TNLM_INVALID_ARG, "TNLM_SWEEP_SHAPE=\"rb,nb\" names a sweep shape that is not available for this window and patch");
     }
     if (geometry) {
         const tnlm_geometry &g = *geometry;
@@ -450,12 +469,10 @@ extern "C" int tnlm_destroy(tnlm_handle *H)
     for (cudaEvent_t e : H->prof_ev) cudaEventDestroy(e);
     free_ws(H);
     if (H->d_scal) cudaFree(H->d_scal);
-    if (H->d_wts) {
-        cudaFree(H->d_wts);
-        // the evict_last lines of the stored weights (apply_resident_mb) would otherwise keep their L2 priority
-        // until something else claims it; ignore a driver that does not support the call
-        if (cudaCtxResetPersistingL2Cache() != cudaSuccess) cudaGetLastError();
-    }
+    // the evict_last lines of the stored weights (apply_resident_mb) keep their L2 priority until other evict_last
+    // traffic claims it: no cudaCtxResetPersistingL2Cache() here, which would also drop the persisting lines of
+    // every other handle and library in the context
+    if (H->d_wts) cudaFree(H->d_wts);
     if (H->d_fbp_g) cudaFree(H->d_fbp_g);
     if (H->d_fbp_cosw) cudaFree(H->d_fbp_cosw);
     if (H->d_fbp_wv) cudaFree(H->d_fbp_wv);
@@ -522,11 +539,17 @@ static int prof_mark(tnlm_handle *H, int kind, bool begin, cudaStream_t st)
     }
     return TNLM_OK;
 }
+// Timing is best effort: a pair whose begin mark failed (event creation or recording) is not recorded at all, and
+// after PROF_MAX_PAIRS undrained pairs (tnlm_kernel_times drains and recycles the events) recording pauses.
+static constexpr size_t PROF_MAX_PAIRS = 1u << 20;
 struct ProfScope {
     tnlm_handle *H;
     cudaStream_t st;
     bool on;
-    ProfScope(tnlm_handle *h, int kind, cudaStream_t s) : H(h), st(s), on(h->prof) { if (on) prof_mark(H, kind, true, st); }
+    ProfScope(tnlm_handle *h, int kind, cudaStream_t s) : H(h), st(s), on(h->prof && h->prof_kind.size() < PROF_MAX_PAIRS)
+    {
+        if (on) on = (prof_mark(H, kind, true, st) == TNLM_OK);
+    }
     ~ProfScope() { if (on) prof_mark(H, 0, false, st); }
 };
 
@@ -535,12 +558,14 @@ struct ProfScope {
 // slice 0) go through the interleaved copies (interleave4_kernel, project_il_kernel, cgls_update_us_il).
 // The strip kernel issues ~1.4x the instructions of the gather kernel (staging, per-chunk extents) and has no
 // memory stalls: measured 12.7 vs 29.0 us on cfg 1 (less than one wave of work: latency bound) and 289 vs 233 us
-// on cfg 4 (issue bound).  Automatic choice: strips while the gather kernel would not fill one wave of CTAs.
+// on cfg 4 (issue bound).  Automatic choice: strips while the gather kernel would have fewer than 2048 ray-threads
+// per SM (one full wave of resident threads).  The crossover is a count of threads, whatever project_block cuts
+// them into: it was measured between cfg 1 (57.6 k rays) and cfg 4 (533 k) and does not move with the CTA size.
 static bool use_strips(const tnlm_handle *H, int n_slices)
 {
     const int nray = H->G.n_views * H->G.n_bins;
-    const long long gather_ctas = (long long)((nray + 255) / 256) * n_slices * H->n_phase;
-    return H->opt_project == 1 || (H->opt_project < 0 && gather_ctas < (long long)H->n_sm * 8);
+    const long long gather_units = (long long)((nray + 255) / 256) * n_slices * H->n_phase;     // of 256 ray-threads
+    return H->opt_project == 1 || (H->opt_project < 0 && gather_units < (long long)H->n_sm * 8);
 }
 static int il_slices(const tnlm_handle *H, int n_slices)
 {
@@ -1021,8 +1046,8 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     auto in = [&](long long lo, long long hi) { return value >= lo && value <= hi; };
     bool ok = true;
     if (n == "weight_cache_mb") H->opt_cache_mb = value;
-    else if (n == "sweep_rb") H->opt_rb = (int)value;
-    else if (n == "sweep_nb") H->opt_nb = (int)value;
+    else if (n == "sweep_rb") { if ((ok = in(0, 64) && sweep_shape_known(H, (int)value, H->opt_nb))) H->opt_rb = (int)value; }
+    else if (n == "sweep_nb") { if ((ok = in(0, 64) && sweep_shape_known(H, H->opt_rb, (int)value))) H->opt_nb = (int)value; }
     else if (n == "apply_ns") { if ((ok = in(0, AP_NS_MAX))) H->opt_ns = (int)value; }
     else if (n == "apply_kernel") { if ((ok = in(0, 2))) H->opt_apply = (int)value; }
     else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
@@ -1035,7 +1060,7 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     else if (n == "apply_snake") { if ((ok = in(0, 1))) H->opt_snake = (int)value; }
     else if (n == "apply_resident_mb") { if ((ok = in(0, 1 << 20))) H->opt_resident_mb = value; }
     else return fail(H, TNLM_INVALID_ARG, "unknown option: " + n);
-    if (!ok) return fail(H, TNLM_INVALID_ARG, "value out of range for option " + n);
+    if (!ok) return fail(H, TNLM_INVALID_ARG, "value out of range (or, for sweep_rb/sweep_nb, not an available shape) for option " + n);
     return TNLM_OK;
 }
 
@@ -1094,31 +1119,6 @@ extern "C" int tnlm_regularize_step(tnlm_handle *H, const float *g, int m2, floa
     return regularize_device(H, g, m2, f_out, n_slices, (cudaStream_t)stream);
 }
 
-// ------------------------------------------------------------------------------ outer loop
-static int reconstruct_device(tnlm_handle *H, const float *y, const float *w, const float *f0, int k_outer, int m1,
-                              int m2, float *f_out, int n_slices, cudaStream_t st)
-{
-    const size_t n = (size_t)n_slices * H->n_phase * H->nx * H->ny;
-    int rc;
-    if (f0) { if (f_out != f0) CU(H, cudaMemcpyAsync(f_out, f0, n * sizeof(float), cudaMemcpyDeviceToDevice, st)); }
-    else CU(H, cudaMemsetAsync(f_out, 0, n * sizeof(float), st));
-    if (k_outer == 0) return TNLM_OK;
-    if ((rc = need(H, &H->d_g, img_count(H)))) return rc;
-    if (m1 > 0 && (rc = prepare_sqrt_weights(H, w, n_slices, st))) return rc;
-    const float *sw = w ? H->d_sw : nullptr;
-    for (int k = 0; k < k_outer; ++k) {
-        if ((rc = cgls_device(H, f_out, y, sw, m1, H->d_g, n_slices, st))) return rc;      // step 2 (L176)
-        if ((rc = regularize_device(H, H->d_g, m2, f_out, n_slices, st))) return rc;       // steps 3-5
-    }
-    return TNLM_OK;
-}
-
-extern "C" int tnlm_reconstruct(tnlm_handle *H, const float *y, const float *w, const float *f0, int k_outer, int m1,
-                                int m2, float *f_out, int n_slices, void *stream)
-{
-    ENTER(H, "tnlm_reconstruct", n_slices, true);
-    int rc;
-    if (!y || !f_out) return fail(H, TNLM_INVALID_ARG, "y and f_out must not be NULL");
 // ------------------------------------------------------------------------------ TNLM step without allocation
 // tnlm_regularize_step_noalloc (tnlm.h): for callers that cannot cudaMalloc -- HBM fully handed out to someone
 // else's allocator, or other streams that must not be stalled by cudaMalloc's device-wide synchronisation.
@@ -1185,6 +1185,31 @@ extern "C" int tnlm_regularize_step_noalloc(tnlm_handle *H, const float *g, int 
     return TNLM_OK;
 }
 
+// ------------------------------------------------------------------------------ outer loop
+static int reconstruct_device(tnlm_handle *H, const float *y, const float *w, const float *f0, int k_outer, int m1,
+                              int m2, float *f_out, int n_slices, cudaStream_t st)
+{
+    const size_t n = (size_t)n_slices * H->n_phase * H->nx * H->ny;
+    int rc;
+    if (f0) { if (f_out != f0) CU(H, cudaMemcpyAsync(f_out, f0, n * sizeof(float), cudaMemcpyDeviceToDevice, st)); }
+    else CU(H, cudaMemsetAsync(f_out, 0, n * sizeof(float), st));
+    if (k_outer == 0) return TNLM_OK;
+    if ((rc = need(H, &H->d_g, img_count(H)))) return rc;
+    if (m1 > 0 && (rc = prepare_sqrt_weights(H, w, n_slices, st))) return rc;
+    const float *sw = w ? H->d_sw : nullptr;
+    for (int k = 0; k < k_outer; ++k) {
+        if ((rc = cgls_device(H, f_out, y, sw, m1, H->d_g, n_slices, st))) return rc;      // step 2 (L176)
+        if ((rc = regularize_device(H, H->d_g, m2, f_out, n_slices, st))) return rc;       // steps 3-5
+    }
+    return TNLM_OK;
+}
+
+extern "C" int tnlm_reconstruct(tnlm_handle *H, const float *y, const float *w, const float *f0, int k_outer, int m1,
+                                int m2, float *f_out, int n_slices, void *stream)
+{
+    ENTER(H, "tnlm_reconstruct", n_slices, true);
+    int rc;
+    if (!y || !f_out) return fail(H, TNLM_INVALID_ARG, "y and f_out must not be NULL");
     if (k_outer < 0 || m1 < 0 || m2 < 0) return fail(H, TNLM_INVALID_ARG, "k_outer, m1, m2 must be >= 0");
     if ((rc = ensure_ws(H, n_slices))) return rc;
     return reconstruct_device(H, y, w, f0, k_outer, m1, m2, f_out, n_slices, (cudaStream_t)stream);

@@ -212,6 +212,19 @@ def test_slice_groups_share_geometry_bit_identically(T):
                 assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 3)) < STEP_TOL
         else:
             assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg, il)
+    # project_block regroups only the ||q||^2 partial sums of the fused CGLS epilogue: P stays bit-identical, CGLS agrees to
+    # rounding.  64 threads = two warps for the four slices of a group: every slice must still reach its reduction
+    # (a slice that did not would keep its iterate, g = f).
+    for pg, il in [(4, 1), (4, 0), (1, 0)]:
+        tn.set_option(hd, "project_group", pg); tn.set_option(hd, "project_interleave", il)
+        for bt in (64, 128, 256):
+            tn.set_option(hd, "project_block", bt)
+            po = torch.empty_like(sinod); go = torch.empty_like(imgd)
+            tn.project(hd, imgd, po)
+            tn.cgls_step(hd, imgd, sinod, wd, 3, go)
+            assert torch.equal(po, ref["p"]), (pg, il, bt)
+            for s in range(S):
+                assert rel(go[s].cpu().numpy(), ref["g"][s].cpu().numpy()) < 1e-5, (pg, il, bt, s)
 
 
 @pytest.mark.parametrize("B,V,L,sid", [(120, 16, 40, 45.0), (200, 9, 40, 45.0), (66, 40, 6, 14.6), (90, 12, 12, 15.0), (140, 7, 30, 27.5)],
@@ -824,3 +837,9 @@ def test_error_codes_and_launch_count(T):
     with pytest.raises(tn.TnlmError) as ei:
         tn.create(None, 16, 16, 2, 3, 3, 1e13, 0.1)
     assert ei.value.code == 1
+    # a sweep shape that was not compiled is refused when the option is set, not at the next launch
+    for name, bad in (("sweep_rb", 7), ("sweep_nb", 3), ("sweep_rb", -1)):
+        with pytest.raises(tn.TnlmError) as ei:
+            tn.set_option(hn, name, bad)
+        assert ei.value.code == 1 and name in str(ei.value)
+    tn.set_option(hn, "sweep_rb", 8); tn.set_option(hn, "sweep_rb", 0)

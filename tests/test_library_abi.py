@@ -32,7 +32,7 @@ def test_every_declared_symbol_is_exported(tn):
 
 def test_argument_validation_happens_before_any_device_work(tn):
     import numpy as np
-    bad = [dict(nx=0), dict(window=4), dict(patch=2), dict(h=0.0), dict(h=float("nan")), dict(mu=-0.1),
+    bad = [dict(nx=0), dict(window=4), dict(patch=2), dict(h=0.0), dict(h=float("nan")), dict(h=1e-20), dict(mu=-0.1),
            dict(n_phase=0)]
     base = dict(nx=8, ny=8, n_phase=3, window=5, patch=3, h=0.01, mu=0.1)
     for b in bad:
