@@ -44,7 +44,7 @@ struct tnlm_handle {
     int n_sm = 148;
     size_t smem_per_sm = 233472;
     // tuning knobs, read once from the environment at tnlm_create (tnlm_set_option changes them later)
-    long long opt_cache_mb = 16384;
+    long long opt_cache_mb = 0;   // 0 (default): every sweep computes the weights in fp32; > 0: sweeps 2..m2 read stored bf16 weights
     int opt_rb = 0, opt_nb = 0, opt_ns = 0;
     int opt_project = -1;   // 1: project_strip_kernel (shared-memory strips per warp); 0: project_kernel (L1 gathers); -1: by size
     int opt_apply = 2;      // 2: gj_apply3_kernel (CTA per band, shared windows, per-warp cp.async rings); 1: gj_apply2_kernel
@@ -132,7 +132,7 @@ static int cuda_fail(tnlm_handle *h, cudaError_t e, const char *what)
         if (e__ != cudaSuccess) return cuda_fail(h, e__, "kernel launch"); \
     } while (0)
 
-extern "C" const char *tnlm_version(void) { return "tnlm-b200 0.2 (sm_100a)"; }
+extern "C" const char *tnlm_version(void) { return "tnlm-b200 0.3 (sm_100a)"; }
 
 extern "C" const char *tnlm_last_error(const tnlm_handle *h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
@@ -961,22 +961,29 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     return TNLM_OK;
 }
 
-// Weight storage for m2 > 1: 2 bytes x 2 sides x W^2 per pixel of the padded band/tile grid.
-// Returns NULL (recompute every sweep instead) when that exceeds the cap
-// (option weight_cache_mb / TNLM_WEIGHT_CACHE_MB, default 16384; 0 disables).
-static __nv_bfloat16 *weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices)
+// Weight storage for m2 > 1 (opt-in: option weight_cache_mb / TNLM_WEIGHT_CACHE_MB > 0): 2 bytes x 2 sides x W^2 per
+// pixel of the padded band/tile grid.  *wts = NULL (every sweep computes its weights in fp32) when the option is 0,
+// the default, or when the need exceeds it.  An allocation that fails is an error of the call (TNLM_ALLOC_FAILED),
+// not a silent change of path.
+static int weight_cache(tnlm_handle *H, const SweepShape &sh, int n_slices, __nv_bfloat16 **wts)
 {
+    *wts = nullptr;
     SweepParams R = H->R;
     fill_layout(H, sh, R);
     const size_t need = (size_t)n_slices * H->n_phase * 2 * R.nbands * R.tiles_x * H->window * H->window * sh.rb * SW_TW;
-    if (H->opt_cache_mb <= 0 || need * sizeof(__nv_bfloat16) > (size_t)H->opt_cache_mb * 1048576ull) return nullptr;
+    if (H->opt_cache_mb <= 0 || need * sizeof(__nv_bfloat16) > (size_t)H->opt_cache_mb * 1048576ull) return TNLM_OK;
     if (need > H->wts_cap) {
         if (H->d_wts) cudaFree(H->d_wts);
         H->d_wts = nullptr; H->wts_cap = 0;
-        if (cudaMalloc(&H->d_wts, need * sizeof(__nv_bfloat16)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        if (cudaMalloc(&H->d_wts, need * sizeof(__nv_bfloat16)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(H, TNLM_ALLOC_FAILED, "device allocation failed (stored weights: " + std::to_string(need * sizeof(__nv_bfloat16) >> 20) +
+                        " MB; lower weight_cache_mb below that, or set it to 0, to compute the weights in every sweep)");
+        }
         H->wts_cap = need;
     }
-    return H->d_wts;
+    *wts = H->d_wts;
+    return TNLM_OK;
 }
 
 extern "C" int tnlm_fma_peak(double *tflops, void *stream)
@@ -1092,7 +1099,8 @@ static int regularize_device(tnlm_handle *H, const float *g, int m2, float *f_ou
     int which = 0;
     const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
     if (!sh) return TNLM_INVALID_ARG;
-    __nv_bfloat16 *wts = (m2 > 1) ? weight_cache(H, *sh, n_slices) : nullptr;   // weights are those of g for all sweeps (L162)
+    __nv_bfloat16 *wts = nullptr;                    // weights are those of g for all sweeps (L162); stored only on request
+    if (m2 > 1 && (rc = weight_cache(H, *sh, n_slices, &wts))) return rc;
     for (int m = 0; m < m2; ++m) {
         const bool last = (m + 1 == m2);
         float *dst;
@@ -1227,7 +1235,8 @@ extern "C" int tnlm_reserve(tnlm_handle *H, int n_slices, int m1, int m2, int ho
     if (m2 > 1) {
         const SweepShape *sh = pick_shape(H, n_slices * H->n_phase);
         if (!sh) return TNLM_INVALID_ARG;
-        weight_cache(H, *sh, n_slices);              // NULL (over the cap) just means "recompute"
+        __nv_bfloat16 *wts = nullptr;                // NULL (option 0, or over the cap) just means "recompute"
+        if ((rc = weight_cache(H, *sh, n_slices, &wts))) return rc;
     }
     if ((rc = need(H, &H->d_g, img_count(H)))) return rc;
     if (host_entry_points && (rc = need(H, &H->d_f, img_count(H)))) return rc;

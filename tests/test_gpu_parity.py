@@ -13,6 +13,7 @@ pytestmark = pytest.mark.gpu
 
 STEP_TOL = 1e-4
 RECON_TOL = 1e-3
+REGRESSION_TOL = 3e-5    # not north_star's: a few times what the fp32 paths measure (1e-6 .. 9e-6), so that a 10x loss of precision fails
 
 
 def rel(a, b):
@@ -355,10 +356,16 @@ def test_regularize_step_matches_oracle(T, N, ny, nx, W, d, h, mu, m2):
     g[0, 3, 4] = -0.003
     hd = tn.create(None, nx, ny, N, W, d, h, mu)
     out = torch.empty(N, ny, nx, device="cuda")
-    tn.regularize_step(hd, dev(torch, g), m2, out)
     want = oracle.regularize_step(g, W, d, h, mu, m2)
-    assert rel(out.cpu().numpy(), want) < STEP_TOL
-    assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
+    # the default (weights computed in fp32 in every sweep), then for m2 > 1 the opt-in stored bf16 weights
+    for cache_mb in ((0, 16384) if m2 > 1 else (0,)):
+        if cache_mb:
+            tn.set_option(hd, "weight_cache_mb", cache_mb)
+        tn.regularize_step(hd, dev(torch, g), m2, out)
+        assert rel(out.cpu().numpy(), want) < STEP_TOL, cache_mb
+        assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max(), cache_mb
+        if not cache_mb:
+            assert rel(out.cpu().numpy(), want) < REGRESSION_TOL      # measured 1e-6 .. 3e-6
 
 
 def test_regularize_edge_cases(T):
@@ -428,6 +435,7 @@ def test_both_stored_weight_sweep_kernels_agree(T):
         g = noisy_stack(N, ny, nx, seed=91)
         gd = dev(torch, g)
         hd = tn.create(None, nx, ny, N, W, d, h, mu)
+        tn.set_option(hd, "weight_cache_mb", 16384)
         ref = torch.empty_like(gd)
         tn.set_option(hd, "apply_kernel", 0)
         tn.regularize_step(hd, gd, m2, ref)
@@ -460,11 +468,13 @@ def test_regularize_multi_slice_equals_per_slice(T):
     g = np.stack([noisy_stack(N, ny, nx, 20 + s) for s in range(S)])
     hd = tn.create(None, nx, ny, N, 7, 5, 0.008, 0.2)
     out = torch.empty(S, N, ny, nx, device="cuda")
-    tn.regularize_step(hd, dev(torch, g), 2, out)
-    for s in range(S):
-        one = torch.empty(N, ny, nx, device="cuda")
-        tn.regularize_step(hd, dev(torch, g[s]), 2, one)
-        assert torch.equal(out[s], one)
+    for cache_mb in (0, 16384):                      # default, then stored weights
+        tn.set_option(hd, "weight_cache_mb", cache_mb)
+        tn.regularize_step(hd, dev(torch, g), 2, out)
+        for s in range(S):
+            one = torch.empty(N, ny, nx, device="cuda")
+            tn.regularize_step(hd, dev(torch, g[s]), 2, one)
+            assert torch.equal(out[s], one)
 
 
 def test_config2_full_size_on_sampled_pixels(T):
@@ -525,20 +535,22 @@ def test_stored_weights_on_high_contrast_and_large_valued_images(T):
         gs = (g * scale).astype(np.float32)
         hd = tn.create(None, nx, ny, N, W, d, h, mu)
         out = torch.empty(N, ny, nx, device="cuda")
-        tn.regularize_step(hd, dev(torch, gs), m2, out)
         want = oracle.regularize_step(gs, W, d, h, mu, m2)
-        assert torch.isfinite(out).all()
-        assert rel(out.cpu().numpy(), want) < STEP_TOL
-        assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
+        for cache_mb in (16384, 0):
+            tn.set_option(hd, "weight_cache_mb", cache_mb)
+            tn.regularize_step(hd, dev(torch, gs), m2, out)
+            assert torch.isfinite(out).all()
+            assert rel(out.cpu().numpy(), want) < STEP_TOL
+            assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
 
 
-def test_stored_weight_rounding_bound_on_binary_images(T):
-    # The documented limit of the stored-weight path (tnlm.h "Stored weights"): a bf16 weight is off by up to 2^-9
-    # relative, which moves a side's weighted mean A/Z by at most 2^-8 x (spread of u_j in the window), i.e. a sweep's
-    # result by at most mu/(2 mu + 2) x 2^-7 x spread.  Binary images of 100 % contrast with a sharp softmax and a
-    # large mu are the worst case: there the stored path misses the 1e-4 bar of BASELINE.json (2e-4 relative L2
-    # measured) while staying inside its own bound; weight_cache_mb = 0 (weights recomputed in fp32 every sweep)
-    # meets 1e-5 on the same input.  (On the thorax-like configs the stored path is at 2e-6: see the headline test.)
+def test_default_path_meets_the_step_bar_on_binary_images_and_the_stored_path_its_own_bound(T):
+    # Binary images of 100 % contrast with a sharp softmax and a large mu are the worst case for rounded weights.
+    # DEFAULT path (no option set: every sweep computes its weights in fp32): north_star's 1e-4 per step, and 1e-5
+    # as a regression bar (1e-6 measured).  OPT-IN stored weights (weight_cache_mb > 0; tnlm.h "Stored weights"): a bf16
+    # weight is off by up to 2^-9 relative, which moves a side's weighted mean A/Z by at most 2^-8 x (spread of u_j
+    # in the window), i.e. a sweep's result by at most mu/(2 mu + 2) x 2^-7 x spread; here it measures 2e-4 relative
+    # L2 -- above the 1e-4 bar, which is why that path is not the default -- and must stay inside its own bound.
     torch, tn = T
     rng = np.random.default_rng(77)
     N, ny, nx, W, d, h, mu, m2 = 2, 60, 130, 7, 3, 0.004, 10.0, 5
@@ -546,14 +558,36 @@ def test_stored_weight_rounding_bound_on_binary_images(T):
     want = oracle.regularize_step(g, W, d, h, mu, m2)
     hd = tn.create(None, nx, ny, N, W, d, h, mu)
     out = torch.empty(N, ny, nx, device="cuda")
+    tn.profile_kernels(hd, True)
+    tn.regularize_step(hd, dev(torch, g), m2, out)                      # as shipped
+    assert [k for k, _ in tn.kernel_times(hd)] == ["sweep"] * m2
+    tn.profile_kernels(hd, False)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+    assert rel(out.cpu().numpy(), want) < REGRESSION_TOL
+    assert np.abs(out.cpu().numpy() - want).max() < 1e-5 * np.abs(want).max()
+    tn.set_option(hd, "weight_cache_mb", 16384)
     tn.regularize_step(hd, dev(torch, g), m2, out)
     spread = float(g.max() - g.min())
     assert np.abs(out.cpu().numpy() - want).max() < mu / (2 * mu + 2) * 2.0 ** -7 * spread
     assert rel(out.cpu().numpy(), want) < 5e-4
-    tn.set_option(hd, "weight_cache_mb", 0)
+
+
+@pytest.mark.parametrize("W,d,mu,h", [(3, 1, 100.0, 0.002), (5, 3, 2.0, 0.004), (7, 5, 10.0, 0.004), (9, 3, 0.5, 0.003),
+                                      (11, 5, 100.0, 0.006), (15, 7, 2.0, 0.005), (21, 3, 10.0, 0.004), (31, 9, 100.0, 0.01)])
+def test_default_path_on_adversarial_binary_images(T, W, d, mu, h):
+    # The sweep that found the stored-weight limit in round 2, as a seeded test of the path as shipped (no option
+    # set): binary images of 100 % contrast plus a little noise, mu-hat from 0.5 to 100, windows from 3 to the compiled
+    # maximum 31, several sweeps, against the oracle at north_star's 1e-4 per step.
+    torch, tn = T
+    rng = np.random.default_rng(1000 + W)
+    N, ny, nx, m2 = 2, 36, 70, 4
+    g = (0.02 * (rng.random((N, ny, nx)) > 0.5) + rng.normal(0, 0.001, (N, ny, nx))).astype(np.float32)
+    want = oracle.regularize_step(g, W, d, h, mu, m2)
+    hd = tn.create(None, nx, ny, N, W, d, h, mu)
+    out = torch.empty(N, ny, nx, device="cuda")
     tn.regularize_step(hd, dev(torch, g), m2, out)
-    assert rel(out.cpu().numpy(), want) < 1e-5
-    assert np.abs(out.cpu().numpy() - want).max() < 1e-5 * np.abs(want).max()
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+    assert np.abs(out.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
 
 
 def test_interleaved_handles_with_different_windows(T):
@@ -734,7 +768,8 @@ def test_config4_size_cgls_and_reconstruct_match_oracle(T):
     out = torch.empty_like(g)
     tn.reconstruct(h, yd, wd, None, 3, cfg.m1, cfg.m2, out)
     want = oracle.reconstruct(og, y, w, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 3, cfg.m1, cfg.m2)
-    assert rel(out.cpu().numpy(), want) < 3 * STEP_TOL
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+    assert rel(out.cpu().numpy(), want) < REGRESSION_TOL
 
 
 def test_twenty_outer_iterations_sharp_softmax_within_1e3(T):
@@ -762,7 +797,8 @@ def test_config3_one_outer_iteration_matches_oracle(T):
     out = torch.empty(cfg.N, cfg.L, cfg.L, device="cuda")
     tn.reconstruct(h, dev(torch, y), dev(torch, w), None, 1, cfg.m1, cfg.m2, out)
     want = oracle.reconstruct(og, y, w, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 1, cfg.m1, cfg.m2)
-    assert rel(out.cpu().numpy(), want) < 3 * STEP_TOL
+    assert rel(out.cpu().numpy(), want) < STEP_TOL
+    assert rel(out.cpu().numpy(), want) < REGRESSION_TOL
 
 
 def test_config5_batch_of_64_slices_matches_oracle_on_three_slices(T):
@@ -781,7 +817,8 @@ def test_config5_batch_of_64_slices_matches_oracle_on_three_slices(T):
     want = oracle.reconstruct(og, y3, w3, None, cfg.L, cfg.L, cfg.window, cfg.patch, cfg.h, cfg.mu, 1, cfg.m1, cfg.m2)
     got = out[pick].cpu().numpy()
     for a in range(3):
-        assert rel(got[a], want[a]) < 3 * STEP_TOL, pick[a]
+        assert rel(got[a], want[a]) < STEP_TOL, pick[a]
+        assert rel(got[a], want[a]) < REGRESSION_TOL, pick[a]
     alone = torch.empty(3, cfg.N, cfg.L, cfg.L, device="cuda")
     tn.reconstruct(h, dev(torch, y3), dev(torch, w3), None, 1, cfg.m1, cfg.m2, alone)
     assert torch.equal(alone, out[pick])
@@ -812,7 +849,14 @@ def test_binding_checks_every_tensor_argument(T):
     tn.profile_kernels(h, False)
     assert kinds == (["transpose", "project", "backproject"] + ["transpose", "project", "cgls_vector", "backproject", "cgls_vector"]
                      + ["project", "cgls_vector", "backproject", "cgls_vector"] + ["project", "cgls_vector"]
-                     + ["sweep_store", "apply", "apply"])
+                     + ["sweep", "sweep", "sweep"])
+    tn.set_option(h, "weight_cache_mb", 16384)           # opt-in stored weights: one storing sweep, then streams
+    tn.reserve(h, 1, cfg.m1, 3, True)
+    tn.profile_kernels(h, True)
+    tn.reconstruct(h, sino, None, None, 1, cfg.m1, 3, img)
+    kinds = [k for k, _ in tn.kernel_times(h)]
+    tn.profile_kernels(h, False)
+    assert kinds[-3:] == ["sweep_store", "apply", "apply"]
 
 
 def test_error_codes_and_launch_count(T):

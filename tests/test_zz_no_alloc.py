@@ -47,13 +47,14 @@ def noisy_stack(N, ny, nx, seed, sigma=0.002):
 
 
 def existing_path(torch, tn, h, gd, m2):
-    """tnlm_regularize_step twice: as shipped (stored bf16 weights for m2 > 1) and with the fp32-recompute switch."""
+    """tnlm_regularize_step twice: with the opt-in stored bf16 weights (sweeps 2..m2 stream them) and as shipped
+    (every sweep computes its weights in fp32)."""
     stored = torch.empty_like(gd)
+    tn.set_option(h, "weight_cache_mb", 16384)
     tn.regularize_step(h, gd, m2, stored)
     tn.set_option(h, "weight_cache_mb", 0)
     fp32 = torch.empty_like(gd)
     tn.regularize_step(h, gd, m2, fp32)
-    tn.set_option(h, "weight_cache_mb", 16384)
     return stored, fp32
 
 
@@ -79,8 +80,8 @@ def test_two_calls_in_a_row_match_the_existing_path(T):
     torch.cuda.synchronize()
     for out, (g, gd, hd, m2, stored, fp32, (W, d, h, mu)) in zip(outs, prepared):
         assert torch.isfinite(out).all()
-        assert rel(out.cpu().numpy(), stored.cpu().numpy()) < STEP_TOL      # vs the path as shipped
-        assert torch.equal(out, fp32)                                       # same kernels, same order: same bits
+        assert rel(out.cpu().numpy(), stored.cpu().numpy()) < STEP_TOL      # vs the stored-weight path
+        assert torch.equal(out, fp32)                                       # vs the path as shipped: same kernels, same bits
         assert rel(out.cpu().numpy(), oracle.regularize_step(g, W, d, h, mu, m2)) < STEP_TOL
     # in place (f_out aliases g), m2 = 1 and m2 = 0 behave like the existing call
     g, gd, hd, m2, stored, fp32, _ = prepared[1]
