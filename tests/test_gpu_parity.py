@@ -255,6 +255,108 @@ def test_backprojector_candidate_range_misses_no_ray(T, B, V, L, sid):
         tn.backproject(h, e.view(1, cfg.V, cfg.B), row.view(1, cfg.L, cfg.L))
         assert torch.equal(row, cols[:, q].contiguous()), int(q)
 
+# --------------------------------------------------------------- the geometry arguments the ABI takes
+def _angles(kind, N, V, rng):
+    """[N][V] source angles: 'random' = unequally spaced, unsorted; 'wild' = repeated, negative and > 2 pi as well."""
+    if kind == "equal":
+        return workloads.view_angles(N, V)
+    a = rng.uniform(0.0, 2.0 * np.pi, size=(N, V))
+    if kind == "wild":
+        a[0, 1] = a[0, 0]                      # a view measured twice in one phase
+        a[-1, 0] = a[0, 0]                     # ... and the same angle again in another phase
+        a[0, 2] -= 2.0 * np.pi                 # negative
+        a[-1, 1] += 4.0 * np.pi                # beyond one turn
+        a[0, 3] = -7.5
+    return a
+
+
+GEOMETRY_CASES = {
+    # ny, nx, N, V, B, pixel_mm, bin_pitch_mm, bin_offset, sid_mm, sdd_mm, angles
+    "wide96x40_pitch1.0239_off0.25": (40, 96, 2, 21, 120, 1.0239, 1.0239, 0.25, 110.0, 190.0, "random"),
+    "tall40x96_pix0.8_off-1.5":      (96, 40, 3, 17, 140, 0.8, 1.1, -1.5, 95.0, 170.0, "wild"),
+    "ragged37x150_off0.25":          (37, 150, 2, 25, 200, 1.0, 1.0, 0.25, 160.0, 260.0, "equal"),
+    "square64_paper_detector":       (64, 64, 2, 19, 96, 1.0, 1.0239, -0.5, 541.0, 949.075, "wild"),
+}
+
+
+@pytest.mark.parametrize("case", sorted(GEOMETRY_CASES))
+def test_projector_family_over_the_geometry_arguments(T, case):
+    # tnlm_geometry takes pixel_mm, bin_offset and arbitrary angles_rad, and tnlm_create takes nx != ny (the paper's own
+    # detector pitch is 1.0239 mm against 1 mm pixels, PAPER.md:L212): every entry point of the projector family
+    # against the oracle on non-square images in both orientations, pixel sizes and detector shifts other than 1 and 0,
+    # and unequally spaced, repeated, negative and > 2 pi source angles.  Five slices: four through the interleaved
+    # forward path, one through the transposed copy.
+    from oracle import fbp
+    torch, tn = T
+    ny, nx, N, V, B, pix, pitch, off, sid, sdd, kind = GEOMETRY_CASES[case]
+    rng = np.random.default_rng(sum(map(ord, case)))
+    ang = _angles(kind, N, V, rng)
+    kw = dict(n_views=V, n_bins=B, sid_mm=sid, sdd_mm=sdd, bin_pitch_mm=pitch, bin_offset=off, pixel_mm=pix, angles_rad=ang)
+    hd = tn.create(tn.Geometry(**kw), nx, ny, N, 5, 3, 0.01, 0.2)
+    og = oracle.Geometry(**kw)
+    f32 = lambda a: a.astype(np.float32).astype(np.float64)
+    S = 5
+    img = rng.random((S, N, ny, nx)) * 0.02; sino = rng.random((S, N, V, B)); w = rng.random((S, N, V, B)) * 50 + 1
+    imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
+    po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
+    tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo); tn.cgls_step(hd, imgd, sinod, wd, 3, go)
+    for s_ in (0, 4):
+        for got, want in ((po[s_], oracle.project(og, f32(img[s_]))),
+                          (bo[s_], oracle.backproject(og, f32(sino[s_]), nx, ny)),
+                          (go[s_], oracle.cgls_step(og, f32(img[s_]), f32(sino[s_]), f32(w[s_]), 3))):
+            assert rel(got.cpu().numpy(), want) < STEP_TOL, (case, s_)
+            assert rel(got.cpu().numpy(), want) < REGRESSION_TOL, (case, s_)
+    # single-slice kernels (strip and gather forward projectors) give the batch's bits
+    for pk in (0, 1):
+        tn.set_option(hd, "project_kernel", pk)
+        one = torch.empty(N, V, B, device="cuda")
+        tn.project(hd, imgd[4].contiguous(), one)
+        assert torch.equal(one, po[4]), (case, pk)
+    tn.set_option(hd, "project_kernel", -1)
+    # adjoint identity on this geometry
+    lhs = (po.double() * sinod.double()).sum().item(); rhs = (imgd.double() * bo.double()).sum().item()
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs)
+    # FBP start (all views of all phases, trapezoid view weights: repeated angles get their share) and two outer
+    # iterations from it, on a sinogram of a smooth object so that the FBP image is not noise
+    yy, xx = np.meshgrid((np.arange(ny) - 0.5 * (ny - 1)) / ny, (np.arange(nx) - 0.5 * (nx - 1)) / nx, indexing="ij")
+    obj = np.stack([0.02 * ((xx / 0.35) ** 2 + (yy / 0.3) ** 2 < 1.0) + 0.01 * (((xx - 0.1 * i) / 0.1) ** 2 + (yy / 0.12) ** 2 < 1.0)
+                    for i in range(N)])
+    y = f32(oracle.project(og, obj))
+    f0 = torch.empty(N, ny, nx, device="cuda")
+    tn.fbp_init(hd, dev(torch, y), f0)
+    want0 = fbp.fbp_init(og, y, nx, ny)
+    assert rel(f0.cpu().numpy(), want0) < STEP_TOL, case
+    assert np.abs(f0.cpu().numpy() - want0).max() < 1e-4 * np.abs(want0).max(), case
+    out = torch.empty(N, ny, nx, device="cuda")
+    tn.reconstruct(hd, dev(torch, y), None, f0, 2, 3, 1, out)
+    want = oracle.reconstruct(og, y, None, f32(f0.cpu().numpy()), nx, ny, 5, 3, 0.01, 0.2, 2, 3, 1)
+    assert rel(out.cpu().numpy(), want) < STEP_TOL, case
+    assert rel(out.cpu().numpy(), want) < REGRESSION_TOL, case
+
+
+@pytest.mark.parametrize("ny,nx", [(5, 9), (9, 5)])
+def test_gpu_projector_matrix_symmetric_entrywise_on_a_shifted_non_square_geometry(T, ny, nx):
+    # The entry-by-entry test of P against P^T, with nx != ny, pixel_mm = 1.0239, bin_offset = 0.25 and unequal angles.
+    torch, tn = T
+    V, B = 6, 16
+    ang = np.array([[0.3, 1.1, 2.9, 3.0, 4.4, 5.9]])
+    kw = dict(n_views=V, n_bins=B, sid_mm=22.0, sdd_mm=38.0, bin_pitch_mm=1.3, bin_offset=0.25, pixel_mm=1.0239, angles_rad=ang)
+    h = tn.create(tn.Geometry(**kw), nx, ny, 1, 3, 3, 0.01, 0.1)
+    og = oracle.Geometry(**kw)
+    npx, nr = ny * nx, V * B
+    cols = torch.empty(npx, nr, device="cuda"); rows = torch.empty(nr, npx, device="cuda")
+    for p in range(npx):
+        e = torch.zeros(npx, device="cuda"); e[p] = 1.0
+        tn.project(h, e.view(1, ny, nx).contiguous(), cols[p].view(1, V, B))
+    for q in range(nr):
+        e = torch.zeros(nr, device="cuda"); e[q] = 1.0
+        tn.backproject(h, e.view(1, V, B).contiguous(), rows[q].view(1, ny, nx))
+    assert torch.equal(cols.t().contiguous(), rows)
+    A = np.stack([oracle.project(og, np.eye(npx)[p].reshape(1, ny, nx)).ravel() for p in range(npx)], axis=1)
+    assert np.abs(rows.cpu().numpy() - A).max() < 2e-5
+    assert (A != 0).sum() > nr                      # the rays do cross the image
+
+
 # ------------------------------------------------------------------------------- random shapes
 def test_random_shapes_match_oracle(T):
     # Seeded random shapes and parameters (image sizes with ragged tiles, every window / patch size, one to three
@@ -298,6 +400,32 @@ def test_random_shapes_match_oracle(T):
         # (fp32 ray tables: 1e-6 typical, up to 1e-5 when a pixel sums only a handful of rays -- 3 views x 10 bins)
         assert rel(po[s].cpu().numpy(), oracle.project(og, f32(img[s]))) < 3e-5, key
         assert rel(bo[s].cpu().numpy(), oracle.backproject(og, f32(sino[s]), L, L)) < 3e-5, key
+        assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, f32(img[s]), f32(sino[s]), f32(w[s]), m1)) < STEP_TOL, key
+        hd.close()
+    # the same over the rest of tnlm_geometry's arguments: nx != ny, pixel_mm != 1, bin_offset != 0, arbitrary angles
+    for _ in range(20):
+        ny = int(rng.integers(5, 70)); nx = ny if rng.random() < 0.3 else int(rng.integers(5, 70))
+        N = int(rng.integers(1, 4)); V = int(rng.integers(3, 40)); B = 2 * int(rng.integers(4, 70))
+        S = int(rng.integers(1, 7)); m1 = int(rng.integers(0, 4))
+        pix = float(rng.uniform(0.5, 1.6)); off = float(rng.uniform(-2.0, 2.0))
+        half_diag = 0.5 * pix * float(np.hypot(nx, ny))
+        sid = half_diag * float(rng.uniform(1.0001, 4.0)) + 6.01 * pix; sdd = sid * float(rng.uniform(1.2, 2.0))
+        pitch = pix * float(rng.uniform(0.5, 2.0))
+        ang = rng.uniform(-2.0 * np.pi, 4.0 * np.pi, size=(N, V)) if rng.random() < 0.7 else workloads.view_angles(N, V)
+        kw = dict(n_views=V, n_bins=B, sid_mm=sid, sdd_mm=sdd, bin_pitch_mm=pitch, bin_offset=off, pixel_mm=pix, angles_rad=ang)
+        try:
+            hd = tn.create(tn.Geometry(**kw), nx, ny, N, 3, 3, 0.01, 0.1)
+        except tn.TnlmError:               # a fan of 180 degrees or more: refused, not wrong
+            continue
+        og = oracle.Geometry(**kw)
+        img = rng.random((S, N, ny, nx)) * 0.02; sino = rng.random((S, N, V, B)); w = rng.random((S, N, V, B)) * 50 + 1
+        imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
+        po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
+        tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo); tn.cgls_step(hd, imgd, sinod, wd, m1, go)
+        s = int(rng.integers(0, S))
+        key = (ny, nx, N, V, B, S, m1, sid, sdd, pitch, pix, off)
+        assert rel(po[s].cpu().numpy(), oracle.project(og, f32(img[s]))) < 3e-5, key
+        assert rel(bo[s].cpu().numpy(), oracle.backproject(og, f32(sino[s]), nx, ny)) < 3e-5, key
         assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, f32(img[s]), f32(sino[s]), f32(w[s]), m1)) < STEP_TOL, key
         hd.close()
 
