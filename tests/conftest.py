@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+    config.addinivalue_line("markers", "slow: minutes of CPU oracle time; runs only with TNLM_FULL_RUN=1")
 
 
 def pytest_collection_modifyitems(config, items):
