@@ -60,25 +60,23 @@
  *   not the default.  If the stored weights cannot be allocated the call fails with TNLM_ALLOC_FAILED.
  *   Options, read from the environment ONCE at tnlm_create and changed later with tnlm_set_option:
  *   weight_cache_mb / TNLM_WEIGHT_CACHE_MB (default 0 = never store; n > 0 = store when the weights of
- *   the call fit in n MB, e.g. 16384; larger needs recompute), sweep_rb, sweep_nb / TNLM_SWEEP_SHAPE="rb,nb" and
- *   apply_ns / TNLM_APPLY_NS=n (restrict the launch-shape heuristics; experiments).  Options without an
- *   environment variable (kernel variants kept for comparison; results are bit-identical either way):
- *   apply_kernel (2 = one CTA per stored band, both windows shared, one cp.async ring per warp: the default;
- *   1 = persistent warp tasks with private windows; 0 = one CTA per band with a TMA ring), apply_depth (ring depth of
- *   kernels 1 and 2; 0 = chosen by the library), apply_wpc (warps per CTA of kernel 1; 0 = cost model),
- *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers),
- *   apply_snake (1, the default: successive stored-weight sweeps deal their tasks in opposite orders, so a sweep
- *   starts on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored
- *   weights are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first;
+ *   the call fit in n MB, e.g. 16384; larger needs recompute) and sweep_rb, sweep_nb / TNLM_SWEEP_SHAPE="rb,nb"
+ *   (pin the launch shape of the sweep instead of the cost model's choice; 0 = free; values that name no
+ *   compiled shape are refused).  Options without an environment variable (results are bit-identical either
+ *   way): apply_depth (ring depth of the stored-weight sweep: 4, 8, 16; 0 = chosen by the library), apply_snake
+ *   (1, the default: successive stored-weight sweeps take the stored bands in opposite orders, so a sweep starts
+ *   on the bytes the previous one left in L2), apply_resident_mb (default 32: that many MB of the stored weights
+ *   are written and read with an L2 evict_last policy, the rest with evict_first; 0 = all evict_first;
  *   tnlm_destroy does not reset the context's persisting L2 lines -- that would hit every other user of the
  *   context -- so those lines keep their priority until other evict_last traffic displaces them),
- *   backproject_group (16, the default; 8, 4, 2, 1) and project_group (1, the default; 2, 4): the slices of one call
- *   share the geometry (nothing couples them, L77), so one thread of a projector serves up to that many slices
- *   with one evaluation of the ray geometry; per slice the arithmetic and its order do not change;
- *   project_interleave (1, the default: in a call with four or more slices the forward projector reads handle-owned
- *   copies of the image in which the four slices of a group are interleaved per pixel, one 16-byte gather per cell
- *   for four slices; 0 = every slice from its own image and transposed copy), project_block (threads per CTA of the
- *   forward projector: 128, the default, 256 or 64; changes only how the ||q||^2 partial sums are grouped).
+ *   project_kernel (-1 = by size, the default; 1 = shared-memory strips per warp; 0 = L1 gathers),
+ *   backproject_group (16, the default; 8, 4, 2, 1): the slices of one call share the geometry (nothing couples
+ *   them, L77), so one backprojector thread serves up to that many slices with one evaluation of the ray
+ *   geometry; per slice the arithmetic and its order do not change; project_interleave (1, the default: in a call
+ *   with four or more slices the forward projector reads handle-owned copies of the image in which the four
+ *   slices of a group are interleaved per pixel, one 16-byte gather per cell for four slices; 0 = every slice
+ *   from its own image and transposed copy), project_block (threads per CTA of the forward projector: 128, the
+ *   default, 256 or 64; changes only how the ||q||^2 partial sums are grouped).
  *
  * Value range
  *   The shifted softmax keeps every weight sum below 2^100, so the numerators sum_delta w u_j stay
@@ -213,8 +211,8 @@ const char *tnlm_last_error(const tnlm_handle *handle);
 int tnlm_reserve(tnlm_handle *handle, int n_slices, int m1, int m2, int host_entry_points);
 
 /* Change a tuning option of this handle (see "Stored weights and tuning knobs"): name is one of
- * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_ns", "apply_kernel", "apply_depth", "apply_wpc",
- * "apply_snake", "apply_resident_mb", "project_kernel", "project_group", "project_interleave", "project_block", "backproject_group"; 0 restores the
+ * "weight_cache_mb", "sweep_rb", "sweep_nb", "apply_depth", "apply_snake", "apply_resident_mb",
+ * "project_kernel", "project_interleave", "project_block", "backproject_group"; 0 restores the
  * heuristic for the shape options.  Unknown names: TNLM_INVALID_ARG. */
 int tnlm_set_option(tnlm_handle *handle, const char *name, long long value);
 

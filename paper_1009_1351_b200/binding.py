@@ -52,8 +52,8 @@ class Geometry:
 
 
 def lib_path() -> str:
-    """The in-tree library; TNLM_LIBRARY names another build of it (kernel experiments)."""
-    return os.environ.get("TNLM_LIBRARY") or os.path.join(_HERE, "libtnlm.so")
+    """The in-tree library, built by `python -m paper_1009_1351_b200.build`."""
+    return os.path.join(_HERE, "libtnlm.so")
 
 
 def library():

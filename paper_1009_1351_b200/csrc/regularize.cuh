@@ -22,7 +22,7 @@
 // about 200/c better than delta = 0) or whose numerator is not below 2^120 is flagged, and flagged
 // pixels are recomputed by the warp with the minimum-subtracted two-pass form (exact_side_ratio)
 // straight from the shared tiles.  With Z < 2^100 the numerator sum_delta e u_j stays finite for
-// |u| < 2^17 (documented in tnlm.h), here and in gj_apply_kernel, which re-reads the same weights.
+// |u| < 2^17 (documented in tnlm.h), here and in gj_apply3_kernel, which re-reads the same weights.
 // The value is always the softmax of Eq. (3); the reference only picks the fp32 range.
 //
 // Borders.  Tiles are zero-filled outside the image (patches are zero-extended, DESIGN.md
@@ -32,7 +32,8 @@
 // outside the image are skipped warp-uniformly.
 //
 // Stored weights ("reusing this factor ... instead of recomputing").  The weights
-// belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 the first sweep
+// belong to g^(k) and stay fixed for all M2 sweeps (L162), so when M2 > 1 and the caller has opted in
+// (option weight_cache_mb > 0; by default every sweep computes its weights) the first sweep
 // (STORE_W = true) also writes every unnormalised weight as bf16 into
 // wts[image][band][tile_x][side][delta][RB/2 row pairs][32 lanes][2 rows][4 columns] -- one
 // contiguous chunk per warp band, written and later read as a sequential stream (DRAM-page
@@ -43,7 +44,7 @@
 // reference and sent every moving edge through the slow exact route: 2.6x slower); the quotient
 // A/Z of Eq. (7) does not depend on the per-pixel scale, and the 2^-9 rounding of each weight
 // moves it by < 1e-6 relative.  Pixels on the exact route store their
-// minimum-subtracted weights instead.  Sweeps 2..M2 are gj_apply_kernel: a streaming pass
+// minimum-subtracted weights instead.  Sweeps 2..M2 are gj_apply3_kernel: a streaming pass
 // over the chunks, bound by HBM (2 bytes per weight) instead of by the FP32 pipes.  With M2 = 1
 // nothing is stored.
 #pragma once
@@ -80,9 +81,8 @@ struct SweepParams {
     float z_limit;          // a side whose weight sum is not below this (2^100) is recomputed exactly
     float a_limit;          // ... or whose numerator magnitude is not below this (2^120)
     int clip;               // apply max(.,0) to the output
-    int ap_ns;              // gj_apply_kernel: stages of its bulk-copy ring
-    int n_img;              // gj_apply2_kernel: S*N images in this launch
-    int ap_reverse;         // gj_apply2_kernel: deal the tasks from the last one down (snake order over the sweeps)
+    int n_img;              // gj_apply3_kernel: S*N images in this launch
+    int ap_reverse;         // gj_apply3_kernel: take the stored bands from the last one down (snake order over the sweeps)
     long long res_tasks;    // stored-weight tasks (row pairs, in layout order) below this index are kept in L2
                             // (evict_last) by the storing sweep and the applying sweeps; the rest streams (evict_first)
 };
@@ -468,330 +468,22 @@ gj_sweep_kernel(SweepParams p, const float *__restrict__ g, const float *__restr
     }
 }
 
-// ---- mbarrier / bulk-copy (TMA) primitives used by gj_apply_kernel -----------------------------------
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// global -> shared bulk copy (16-byte aligned, size a multiple of 16), completion counted on bar
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-
-// Sweeps 2..M2 with the stored weights: u_i'(x) = g_i(x)/(1+mu) + mu/(2mu+2) * sum over the two sides of
-// (sum_delta w u_j(x+delta)) / (sum_delta w), w read back as bf16 (2 bytes per weight: HBM bound).
-// CTA = one stored band: p.rb consumer warps (one per row, lane l owns columns 4l..4l+3 of the
-// 128-column tile) + one producer warp.  The band's two chunks are contiguous in memory, so the
-// producer streams them front to back with bulk copies (cp.async.bulk, TMA) of up to AP_SO
-// offsets per stage into an AP_NS-deep shared-memory ring; full/empty mbarriers hand stages
-// over, nothing else synchronises.  u_j of both neighbours is staged with its halo in shared
-// memory, zero-filled outside the image (excluded candidates carry weight 0 in the chunks).
-// grid.x = (S*N) * ceil(ny / rb) * tiles_x; block = 32 * (rb + 1).
-// Measured ceiling (round-1 working notes): streaming the same 322 MB by bulk copies alone, no arithmetic,
-// takes 65 us (4.9 TB/s) for any stage size 2.5-31 KB and ring depth 2-8; a grid-stride LDG.128 read
-// reaches 5.6 TB/s, but an 8-byte-per-lane register-pipelined variant of this kernel ran at 151 us.
-constexpr int AP_SO = 4;         // offsets (consecutive dc of one dr) per stage
-constexpr int AP_NS_MAX = 8;     // stages in flight: p.ap_ns, chosen per launch (wave quantisation vs bytes in flight)
+// ---- sweeps 2..M2 from the stored weights (opt-in, option weight_cache_mb > 0) ---------------------------------
+// u_i'(x) = g_i(x)/(1+mu) + mu/(2mu+2) * sum over the two sides of (sum_delta w u_j(x+delta)) / (sum_delta w), with w
+// read back as bf16: 2 bytes per weight, HBM bound.  One CTA per stored band (chunk) of rb rows x 128 columns; warp k
+// owns the ROW PAIR 2k, 2k+1 (lane l: columns 4l..4l+3 of both rows).  The row-pair interleave of the stored layout
+// (plane_off) makes a warp's share of one offset plane a contiguous piece of 512 bytes, 16 bytes per lane, so the
+// 2 W^2 pieces of a warp (both sides) are one uninterrupted stream with a constant stride, kept DEPTH pieces deep
+// in a private cp.async ring (LDGSTS: no registers held by loads in flight, no mbarriers, no producer warp).  The
+// u_j windows of BOTH sides (rb + 2a rows each, zero-filled outside the image; excluded candidates carry weight 0
+// in the chunks) are staged once by all threads of the CTA.  Measured on the box: a 322 MB
+// read-only stream of this shape runs at 6.2 TB/s; this kernel reaches 5.7-5.8 TB/s (0.87-0.89 of the copy peak).
+// Two earlier formulations were measured and removed in round 3: one CTA per band fed by a producer warp through a
+// cp.async.bulk (TMA) ring with mbarriers (72 us per cfg-2 sweep: bulk copies alone, no arithmetic, streamed the same
+// bytes at 4.9 TB/s for any stage size and depth) and persistent warp tasks with private windows (62 us: two ring
+// restarts per task and 3x the window bytes from L2); this one takes 56-57 us.  All three were bit-identical.
+// grid.x = chunks = (S*N) * bands that hold image rows * tiles_x; block = 32 * rb/2; dynamic smem = apply3_smem_bytes.
 __host__ __device__ inline int apply_uw(int window) { return 124 + 4 * ((window + 3) / 4 + 1); }
-__host__ __device__ inline size_t apply_smem_bytes(int window, int rb, int ns)
-{
-    const int a = (window - 1) / 2;
-    return (size_t)ns * AP_SO * rb * SW_TW * sizeof(__nv_bfloat16) + (size_t)2 * (rb + 2 * a) * apply_uw(window) * sizeof(float) +
-           2 * AP_NS_MAX * sizeof(uint64_t);
-}
-
-__global__ void __launch_bounds__(352)
-gj_apply_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
-                const __nv_bfloat16 *__restrict__ wts)
-{
-    constexpr int C = SW_C;
-    const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1;
-    const int nchunk = (W + 3) >> 2;
-    const int UW = apply_uw(W);                     // lane reads words [4l + 4k, 4l + 4k + 8)
-    const int rb = p.rb, urows = rb + 2 * a;
-    const size_t wstride = (size_t)rb * SW_TW;      // halves per offset
-    extern __shared__ float4 smem4[];
-    const int AP_NS = p.ap_ns;
-    __nv_bfloat16 *sW = reinterpret_cast<__nv_bfloat16 *>(smem4);                   // [AP_NS][AP_SO][rb][128]
-    float *sU = reinterpret_cast<float *>(sW + (size_t)AP_NS * AP_SO * wstride);    // [2][urows][UW]
-    uint64_t *full = reinterpret_cast<uint64_t *>(sU + 2 * urows * UW);             // [AP_NS_MAX], then empty[AP_NS_MAX]
-    uint64_t *empty = full + AP_NS_MAX;
-
-    const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
-    const int img = blockIdx.x / tiles_per_img;
-    const int tl = blockIdx.x - img * tiles_per_img;
-    const int gband = tl / p.tiles_x, tx = tl - gband * p.tiles_x;
-    const int tile_r0 = gband * rb, tile_c0 = tx * SW_TW;
-    const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
-    const size_t npix = (size_t)nx * ny;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-    if (threadIdx.x == 0) {
-        for (int i = 0; i < p.ap_ns; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, rb); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-
-    // stage t = (side, dr, k): offsets dr*W + 4k .. of that side's chunk, min(4, W-4k) of them
-    const int stages_per_side = W * nchunk, T = 2 * stages_per_side;
-    const size_t side_stride = (size_t)(W * W) * wstride;       // the two sides of a band are contiguous
-    const __nv_bfloat16 *__restrict__ chunk0 = wts + ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2) * (size_t)(W * W) * wstride;
-
-    if (warp == rb) {                               // ---- producer warp: one lane issues the bulk copies
-        if (lane == 0) {
-            int slot = 0, round = 0;
-            for (int t = 0; t < T; ++t) {
-                if (round > 0) mbar_wait(empty + slot, (round - 1) & 1);
-                const int sd = t / stages_per_side, rem = t - sd * stages_per_side;
-                const int dr = rem / nchunk, k = rem - dr * nchunk;
-                const int noff = min(AP_SO, W - AP_SO * k);
-                const unsigned bytes = (unsigned)(noff * wstride * sizeof(__nv_bfloat16));
-                mbar_expect_tx(full + slot, bytes);
-                bulk_g2s(sW + (size_t)slot * AP_SO * wstride, chunk0 + sd * side_stride + (size_t)(dr * W + AP_SO * k) * wstride,
-                         bytes, full + slot);
-                if (++slot == AP_NS) { slot = 0; ++round; }
-            }
-        }
-        return;
-    }
-
-    // ---- consumer warps: stage u_j (overlaps the first bulk copies), then drain the ring
-#pragma unroll
-    for (int s = 0; s < 2; ++s) {
-        const int j = (phase + (s == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
-        stage_tile_async(sU + s * urows * UW, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, tile_r0 - a,
-                         tile_c0 - a, ny, nx, warp, rb, lane);
-    }
-    cp_async_commit();
-    cp_async_wait<0>();
-    asm volatile("bar.sync 1, %0;" ::"r"(32 * rb) : "memory");      // consumers only
-
-    const int r = tile_r0 + warp, c0 = tile_c0 + C * lane;
-    float nbsum[C] = {0.f, 0.f, 0.f, 0.f};
-    int slot = 0;
-    unsigned parity = 0;
-#pragma unroll 1
-    for (int s = 0; s < 2; ++s) {
-        float Z[C] = {0.f, 0.f, 0.f, 0.f}, A[C] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll 1
-        for (int dr = 0; dr < W; ++dr) {
-            const float4 *__restrict__ up = reinterpret_cast<const float4 *>(sU + (s * urows + warp + dr) * UW) + lane;
-#pragma unroll 1
-            for (int k = 0; k < nchunk; ++k) {
-                const float4 u0 = up[k], u1 = up[k + 1];
-                const float uw[8] = {u0.x, u0.y, u0.z, u0.w, u1.x, u1.y, u1.z, u1.w};
-                const int noff = min(AP_SO, W - AP_SO * k);
-                mbar_wait(full + slot, parity);
-                const uint2 *__restrict__ wq = reinterpret_cast<const uint2 *>(sW + (size_t)slot * AP_SO * wstride + plane_off(warp, C * lane));
-                uint2 wv[AP_SO];
-#pragma unroll
-                for (int jj = 0; jj < AP_SO; ++jj) wv[jj] = wq[(jj < noff ? jj : 0) * (wstride / 4)];
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty + slot);           // values are in registers: slot is free
-                if (++slot == AP_NS) { slot = 0; parity ^= 1u; }
-#pragma unroll
-                for (int jj = 0; jj < AP_SO; ++jj) {
-                    if (jj < noff) {
-                        const float2 lo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&wv[jj].x));
-                        const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162 *>(&wv[jj].y));
-                        const float w[C] = {lo.x, lo.y, hi.x, hi.y};
-#pragma unroll
-                        for (int c = 0; c < C; ++c) {
-                            Z[c] += w[c];
-                            A[c] = fmaf(w[c], uw[c + jj], A[c]);
-                        }
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < C; ++c) nbsum[c] += A[c] / Z[c];
-    }
-    if (r >= ny || c0 >= nx) return;
-    const float *__restrict__ gi = g + (size_t)img * npix + (size_t)r * nx + c0;
-    float *__restrict__ o = out + (size_t)img * npix + (size_t)r * nx + c0;
-#pragma unroll
-    for (int c = 0; c < C; ++c)
-        if (c0 + c < nx) {
-            float v = fmaf(p.c_nb, nbsum[c], p.c_self * __ldg(gi + c));
-            if (p.clip) v = fmaxf(v, 0.f);
-            o[c] = v;
-        }
-}
-
-// The same sweep as a persistent, warp-task kernel (the default).  A task = one ROW PAIR of one stored band
-// (2 rows x 128 columns, both sides): the 2*W^2 pieces of 512 bytes that hold its weights (the row-pair
-// interleave of the stored layout makes a warp's piece contiguous, 16 bytes per lane).  Tasks are dealt
-// round-robin to all resident warps of the device, so every SM streams the same number of bytes to within one
-// task.  A warp is self-contained: it stages its own u_j window (2+2a rows) and keeps DEPTH pieces in flight in a
-// private ring, all with cp.async (LDGSTS: no registers held by loads in flight, no mbarriers, no producer
-// warp), and never synchronises with another warp.  Measured on the box: a 322 MB
-// read-only stream of this shape runs at 6.2 TB/s; what kept the first versions at 4.4 TB/s was the u_j tile
-// staging (a load-then-store loop: one exposed L2 round trip per row), not the stream.
-// grid.x = resident CTAs (host: n_sm x CTAs per SM); block = 32 x warps per CTA (host's choice);
-// dynamic smem = warps x apply2_warp_bytes.
-__host__ __device__ inline size_t apply2_warp_bytes(int window, int depth)
-{
-    const int a = (window - 1) / 2;
-    return (size_t)(2 + 2 * a) * apply_uw(window) * sizeof(float) + (size_t)depth * 512;
-}
-
-// Tried and dropped: writing the weight sums Z in the first applying sweep and reading them back in the later ones
-// (8 fewer instructions per 512-byte piece) leaves the sweep at the same 61.8 us: it waits for bytes, not for issue slots.
-template <int DEPTH>             // pieces in flight per warp (a power of two)
-__global__ void __launch_bounds__(256, 2)
-gj_apply2_kernel(SweepParams p, const float *__restrict__ g, const float *__restrict__ u, float *__restrict__ out,
-                 const __nv_bfloat16 *__restrict__ wts)
-{
-    constexpr int C = SW_C;
-    const int a = p.a, nx = p.nx, ny = p.ny, W = 2 * a + 1, WW = W * W;
-    const int UW = apply_uw(W), urows = 2 + 2 * a;
-    const int rb = p.rb, npairs = rb >> 1;
-    const size_t pstride = (size_t)rb * (SW_TW / 8);     // uint4 per offset plane
-    const size_t side_stride = (size_t)WW * pstride;     // uint4; the two sides of a band are contiguous
-    const size_t npix = (size_t)nx * ny;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, wpc = blockDim.x >> 5;
-    extern __shared__ float4 smem4[];
-    const size_t wbytes = apply2_warp_bytes(W, DEPTH);
-    float *sU = reinterpret_cast<float *>(reinterpret_cast<char *>(smem4) + warp * wbytes);   // [urows][UW]
-    const unsigned ring_s = smem_u32(sU + urows * UW) + 16 * lane;                           // [DEPTH][32 lanes] x 16 B
-
-    const int tiles_per_img = p.tiles_x * p.tiles_y;       // tiles_y = bands that hold image rows
-    const long long n_tasks = (long long)p.n_img * tiles_per_img * npairs;
-    const long long n_warps = (long long)gridDim.x * wpc;
-    const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
-#pragma unroll 1
-    for (long long base = (long long)blockIdx.x * wpc; base < n_tasks; base += n_warps) {
-        // (the L2 policy is chosen per CTA and round, from `base`: uniform, so it lives in a uniform register)
-        const uint64_t pol = (p.ap_reverse ? n_tasks - 1 - base : base) < p.res_tasks ? pol_keep : pol_stream;
-        const long long tk = base + warp;
-        if (tk >= n_tasks) break;
-        const long long task = p.ap_reverse ? n_tasks - 1 - tk : tk;
-        const int pair = (int)(task % npairs);
-        const long long chunk = task / npairs;               // (img, gband, tx)
-        const int img = (int)(chunk / tiles_per_img);
-        const int tl = (int)(chunk - (long long)img * tiles_per_img);
-        const int gband = tl / p.tiles_x, tx = tl - gband * p.tiles_x;
-        const int r = gband * rb + 2 * pair, tile_c0 = tx * SW_TW, c0 = tile_c0 + C * lane;
-        const int slice = img / p.n_phase, phase = img - slice * p.n_phase;
-        const uint4 *__restrict__ wp = reinterpret_cast<const uint4 *>(wts) +
-                                       ((((size_t)img * p.nbands + gband) * p.tiles_x + tx) * 2) * (size_t)WW * pstride +
-                                       pair * 32 + lane;
-        float nbsum[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-#pragma unroll 1
-        for (int sd = 0; sd < 2; ++sd) {
-            const uint4 *__restrict__ ws = wp + sd * side_stride;
-            const int j = (phase + (sd == 0 ? p.n_phase - 1 : 1)) % p.n_phase;
-            __syncwarp();                                     // the previous window is no longer read
-            // oldest group: this side's u_j window; then pieces 0..DEPTH-2 of its weights
-            stage_tile_async(sU, urows, UW, u + ((size_t)slice * p.n_phase + j) * npix, r - a, tile_c0 - a, ny, nx, 0, 1, lane);
-            cp_async_commit();
-            const uint4 *__restrict__ nextp = ws;             // piece `issued` of this side
-            unsigned issued = 0;
-            // (the write slot is a per-lane running address: with a uniform ring offset ptxas folds it into
-            // [R + UR] addressing, and an LDGSTS that also carries an L2 policy in desc[UR] then faults)
-            unsigned wr = ring_s;
-#pragma unroll 1
-            for (; issued < DEPTH - 1; ++issued, nextp += pstride) {
-                cp_async16_s_hint(wr, nextp, issued < (unsigned)WW, pol);
-                cp_async_commit();
-                wr += 512;
-            }
-            float Z[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, A[2][C] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-            cp_async_wait<DEPTH - 1>();                       // the window has landed (every lane's part of it)
-            __syncwarp();
-            unsigned t = 0;
-#pragma unroll 1
-            for (int dr = 0; dr < W; ++dr) {
-                const float *__restrict__ urow0 = sU + dr * UW + C * lane;
-#pragma unroll 1
-                for (int k = 0; k < W; k += 4) {
-                    const float4 ua = *reinterpret_cast<const float4 *>(urow0 + k), ub = *reinterpret_cast<const float4 *>(urow0 + k + 4);
-                    const float4 uc = *reinterpret_cast<const float4 *>(urow0 + UW + k), ud = *reinterpret_cast<const float4 *>(urow0 + UW + k + 4);
-                    const float uw0[8] = {ua.x, ua.y, ua.z, ua.w, ub.x, ub.y, ub.z, ub.w};
-                    const float uw1[8] = {uc.x, uc.y, uc.z, uc.w, ud.x, ud.y, ud.z, ud.w};
-                    const int noff = min(4, W - k);
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        if (jj < noff) {
-                            cp_async16_s_hint(wr, nextp, issued < (unsigned)WW, pol);
-                            cp_async_commit();                // (empty groups keep the wait count uniform)
-                            ++issued; nextp += pstride;
-                            wr = (wr == ring_s + (DEPTH - 1) * 512) ? ring_s : wr + 512;
-                            cp_async_wait<DEPTH - 1>();       // piece t has landed (this lane's own 16 bytes)
-                            const uint4 wv = lds128_s(ring_s + ((t & (DEPTH - 1)) << 9));
-                            ++t;
-                            // bf16 -> fp32 is a 16-bit shift: low half << 16, high half masked
-                            const float w0[C] = {__uint_as_float(wv.x << 16), __uint_as_float(wv.x & 0xffff0000u),
-                                                 __uint_as_float(wv.y << 16), __uint_as_float(wv.y & 0xffff0000u)};
-                            const float w1[C] = {__uint_as_float(wv.z << 16), __uint_as_float(wv.z & 0xffff0000u),
-                                                 __uint_as_float(wv.w << 16), __uint_as_float(wv.w & 0xffff0000u)};
-#pragma unroll
-                            for (int c = 0; c < C; ++c) {
-                                Z[0][c] += w0[c];
-                                A[0][c] = fmaf(w0[c], uw0[c + jj], A[0][c]);
-                                Z[1][c] += w1[c];
-                                A[1][c] = fmaf(w1[c], uw1[c + jj], A[1][c]);
-                            }
-                        }
-                    }
-                }
-            }
-#pragma unroll
-            for (int c = 0; c < C; ++c) {
-                nbsum[0][c] += A[0][c] / Z[0][c];
-                nbsum[1][c] += A[1][c] / Z[1][c];
-            }
-        }
-        if (c0 < nx) {
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                if (r + q < ny) {
-                    const float *__restrict__ gi = g + (size_t)img * npix + (size_t)(r + q) * nx + c0;
-                    float *__restrict__ o = out + (size_t)img * npix + (size_t)(r + q) * nx + c0;
-#pragma unroll
-                    for (int c = 0; c < C; ++c)
-                        if (c0 + c < nx) {
-                            float v = fmaf(p.c_nb, nbsum[q][c], p.c_self * __ldg(gi + c));
-                            if (p.clip) v = fmaxf(v, 0.f);
-                            o[c] = v;
-                        }
-                }
-            }
-        }
-    }
-}
-
-// The same sweep with one CTA per stored band (chunk): its rb/2 warps (one per row pair) share the u_j windows of
-// BOTH sides (rb + 2a rows each, staged once by all threads), so a warp's 2 W^2 pieces form one uninterrupted
-// stream -- gj_apply2_kernel drains its ring and restages a window between the two sides of every task (two pipeline
-// restarts of ~2.5 us in a 62 us launch, and 3x the window bytes from L2).  Arithmetic and its order are those of
-// gj_apply2_kernel (bit-identical results).  grid.x = chunks = (S*N) * bands that hold image rows * tiles_x;
-// block = 32 * rb/2; dynamic smem = apply3_smem_bytes.
 __host__ __device__ inline size_t apply3_smem_bytes(int window, int rb, int depth)
 {
     const int a = (window - 1) / 2;

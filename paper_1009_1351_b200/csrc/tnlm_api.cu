@@ -45,17 +45,13 @@ struct tnlm_handle {
     size_t smem_per_sm = 233472;
     // tuning knobs, read once from the environment at tnlm_create (tnlm_set_option changes them later)
     long long opt_cache_mb = 0;   // 0 (default): every sweep computes the weights in fp32; > 0: sweeps 2..m2 read stored bf16 weights
-    int opt_rb = 0, opt_nb = 0, opt_ns = 0;
+    int opt_rb = 0, opt_nb = 0;
     int opt_project = -1;   // 1: project_strip_kernel (shared-memory strips per warp); 0: project_kernel (L1 gathers); -1: by size
-    int opt_apply = 2;      // 2: gj_apply3_kernel (CTA per band, shared windows, per-warp cp.async rings); 1: gj_apply2_kernel
-                            // (persistent warp tasks); 0: gj_apply_kernel (CTA per band, TMA ring)
-    int opt_depth = 0;      // gj_apply2_kernel ring depth override (0 = cost model)
-    int opt_wpc = 0;        // gj_apply2_kernel warps per CTA override (0 = cost model)
+    int opt_depth = 0;      // gj_apply3_kernel ring depth override (0 = the deepest of 8, 4 that fits)
     int opt_project_il = 1;         // forward projector: groups of four slices read interleaved copies (project_il_kernel)
     int opt_project_block = 128;    // project_kernel / project_il_kernel: threads per CTA (256, 128, 64; 128 measured 2-3 % faster than 256: tail balance)
-    int opt_project_group = 1;      // project_kernel: at most this many slices of a batch per thread (4, 2 or 1)
-    int opt_backproject_group = 16; // backproject_kernel: the same (16, 8, 4, 2 or 1)
-    int opt_snake = 1;      // gj_apply2_kernel: successive sweeps deal their tasks in opposite orders
+    int opt_backproject_group = 16; // backproject_kernel: at most this many slices of a batch per thread (16, 8, 4, 2 or 1)
+    int opt_snake = 1;      // gj_apply3_kernel: successive sweeps take the stored bands in opposite orders
     long long opt_resident_mb = 32;   // MB of stored weights marked evict_last in L2 (the rest evict_first); 0 = none
     // geometry tables (device)
     RayEntry *d_tab = nullptr;
@@ -331,12 +327,6 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     H->device = dev;
     if (const char *ev = std::getenv("TNLM_WEIGHT_CACHE_MB")) H->opt_cache_mb = std::strtoll(ev, nullptr, 10);
     if (const char *ev = std::getenv("TNLM_SWEEP_SHAPE")) std::sscanf(ev, "%d,%d", &H->opt_rb, &H->opt_nb);
-    if (const char *ev = std::getenv("TNLM_APPLY_NS")) {
-        char *end = nullptr;
-        const long v = std::strtol(ev, &end, 10);
-        if (end == ev || *end || v < 0 || v > AP_NS_MAX) { delete H; return fail(nullptr, TNLM_INVALID_ARG, "TNLM_APPLY_NS must be an integer in [0, " + std::to_string(AP_NS_MAX) + "]"); }
-        H->opt_ns = (int)v;
-    }
 
     // TNLM parameters
     SweepParams &R = H->R;
@@ -354,14 +344,7 @@ extern "C" int tnlm_create(const tnlm_geometry *geometry, int nx, int ny, int n_
     R.clip = 0;
     {
         H->apply_smem = (size_t)prop.sharedMemPerBlockOptin;     // per kernel symbol: always the device maximum
-        ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)H->apply_smem);
-        // ask for the largest shared-memory carveout so that the ring-depth choice below decides the occupancy
-        if (ce == cudaSuccess)
-            ce = cudaFuncSetAttribute((const void *)gj_apply_kernel, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                      cudaSharedmemCarveoutMaxShared);
-        for (const void *fn : {(const void *)gj_apply2_kernel<4>, (const void *)gj_apply2_kernel<8>, (const void *)gj_apply2_kernel<16>,
-                               (const void *)gj_apply3_kernel<4>, (const void *)gj_apply3_kernel<8>, (const void *)gj_apply3_kernel<16>})
+        for (const void *fn : {(const void *)gj_apply3_kernel<4>, (const void *)gj_apply3_kernel<8>, (const void *)gj_apply3_kernel<16>})
             if (ce == cudaSuccess) ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)H->apply_smem);
         if (ce != cudaSuccess) { delete H; return cuda_fail(nullptr, ce, "apply kernel setup"); }
     }
@@ -618,20 +601,12 @@ static int launch_project(tnlm_handle *H, const float *img, bool copies_ready, c
                                                        reinterpret_cast<const float4 *>(H->d_imT), y, sw, out0, out1, red);
         LAUNCHED(H);
     }
-    // the other slices from the image and its transpose, up to project_group slices per thread (project_kernel)
-    const int max_ns = H->opt_project_group;
-    int s0 = n_il;
-    for (int ns = 4; ns >= 1; ns >>= 1) {
-        if (ns > max_ns) continue;
-        const int groups = (n_slices - s0) / ns;
-        if (groups < 1) continue;
+    // the other slices (fewer than four, or the remainder of a batch) one per thread from the image and its transpose
+    if (n_slices > n_il) {
         const int bt = H->opt_project_block;             // threads per CTA (256, 128 or 64)
-        dim3 grid((nray + bt - 1) / bt, groups * H->n_phase);
-        if (ns == 4) project_kernel<MODE, 4><<<grid, bt, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
-        else if (ns == 2) project_kernel<MODE, 2><<<grid, bt, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
-        else project_kernel<MODE, 1><<<grid, bt, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, s0);
+        dim3 grid((nray + bt - 1) / bt, (n_slices - n_il) * H->n_phase);
+        project_kernel<MODE, 1><<<grid, bt, 0, st>>>(H->G, H->d_tab, H->d_rng, img, imgT, y, sw, out0, out1, red, n_il);
         LAUNCHED(H);
-        s0 += groups * ns;
     }
     return TNLM_OK;
 }
@@ -882,81 +857,19 @@ static int launch_apply(tnlm_handle *H, const SweepShape &sh, const float *g, co
     R.tiles_y = (H->ny + sh.rb - 1) / sh.rb;             // CTA = one band that holds image rows
     const long long ctas = (long long)n_slices * H->n_phase * R.tiles_x * R.tiles_y;
     if (ctas > 2147483647LL) return fail(H, TNLM_UNSUPPORTED, "too many tiles for one launch");
-    if (H->opt_apply == 2) {
-        // one CTA per band, the windows of both sides shared by its warps (gj_apply3_kernel)
-        R.n_img = n_slices * H->n_phase;
-        int dp = H->opt_depth ? H->opt_depth : 8;
-        while (dp > 4 && apply3_smem_bytes(H->window, sh.rb, dp) > H->apply_smem) dp >>= 1;
-        const size_t sm = apply3_smem_bytes(H->window, sh.rb, dp);
-        if (sm > H->apply_smem) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
-        const unsigned threads = 32u * (unsigned)(sh.rb / 2);
-        ProfScope ps(H, TNLM_KERNEL_APPLY, st);
-        switch (dp) {
-            case 16: gj_apply3_kernel<16><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
-            case 8: gj_apply3_kernel<8><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
-            default: gj_apply3_kernel<4><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
-        }
-        LAUNCHED(H);
-        return TNLM_OK;
-    }
-    if (H->opt_apply == 1) {
-        // Persistent warp tasks (row pairs).  Launch shape by a small cost model: for every ring depth and CTA
-        // size, the resident warps W and the bytes they keep in flight bound the rate of a round at
-        // min(6.2 TB/s, in-flight / 1.5 us); tasks / W full rounds, then one round with the remaining tasks.
-        R.n_img = n_slices * H->n_phase;
-        const long long tasks = ctas * (sh.rb / 2);
-        const double task_bytes = 2.0 * H->window * H->window * 512.0;
-        int best_dp = 0, best_wpc = 0, best_per_sm = 0;
-        double best_t = 0.0;
-        for (int dp = 16; dp >= 4; dp >>= 1) {
-            if (H->opt_depth && dp != H->opt_depth) continue;                      // tuning overrides
-            const size_t wb = apply2_warp_bytes(H->window, dp);
-            for (int wpc = 8; wpc >= 2; --wpc) {
-                if (H->opt_wpc && wpc != H->opt_wpc) continue;
-                const size_t need = wpc * wb;
-                if (need > H->apply_smem) continue;
-                const int per_sm = (int)std::min<size_t>(H->smem_per_sm / (need + 1024), (size_t)(20 / wpc));   // 94 registers: 20 warps per SM
-                if (per_sm < 1) continue;
-                const long long warps = std::min<long long>((long long)H->n_sm * per_sm * wpc, tasks);
-                auto round_time = [&](long long active) {
-                    const double rate = std::min(6.2e12, (double)active * (dp - 1) * 512.0 / 1.5e-6);
-                    return (double)active * task_bytes / rate;
-                };
-                double t = (double)(tasks / warps) * round_time(warps);
-                if (tasks % warps) t += round_time(tasks % warps);
-                if (!best_dp || t < best_t * 0.999) { best_dp = dp; best_wpc = wpc; best_per_sm = per_sm; best_t = t; }
-            }
-        }
-        if (!best_dp) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
-        const long long want = (tasks + best_wpc - 1) / best_wpc;
-        const unsigned grid = (unsigned)std::min<long long>((long long)H->n_sm * best_per_sm, want);
-        const size_t sm = best_wpc * apply2_warp_bytes(H->window, best_dp);
-        ProfScope ps(H, TNLM_KERNEL_APPLY, st);
-        switch (best_dp) {
-            case 16: gj_apply2_kernel<16><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
-            case 8: gj_apply2_kernel<8><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
-            default: gj_apply2_kernel<4><<<grid, 32 * best_wpc, sm, st>>>(R, g, u, out, wts); break;
-        }
-        LAUNCHED(H);
-        return TNLM_OK;
-    }
-    // ring depth: the most stages whose shared memory still leaves the last wave best filled
-    const int threads = 32 * (sh.rb + 1);
-    double best_eff = -1.0;
-    size_t smem = 0;
-    for (int ns = AP_NS_MAX; ns >= 2; --ns) {
-        if (H->opt_ns && ns != H->opt_ns) continue;      // tuning override
-        const size_t sm = apply_smem_bytes(H->window, sh.rb, ns);
-        if (sm > H->apply_smem) continue;
-        const long long occ = std::min<long long>((long long)(H->smem_per_sm / (sm + 1024)), 2048 / threads);
-        if (occ < 1) continue;
-        const long long cap = occ * H->n_sm, waves = (ctas + cap - 1) / cap;
-        const double eff = (double)ctas / (double)(waves * cap) - 1e-3 * (double)waves + 1e-5 * ns;   // ties: fewer waves, then deeper ring
-        if (eff > best_eff) { best_eff = eff; R.ap_ns = ns; smem = sm; }
-    }
-    if (best_eff < 0.0) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+    // one CTA per stored band, the windows of both sides shared by its warps (gj_apply3_kernel)
+    R.n_img = n_slices * H->n_phase;
+    int dp = H->opt_depth ? H->opt_depth : 8;
+    while (dp > 4 && apply3_smem_bytes(H->window, sh.rb, dp) > H->apply_smem) dp >>= 1;
+    const size_t sm = apply3_smem_bytes(H->window, sh.rb, dp);
+    if (sm > H->apply_smem) return fail(H, TNLM_UNSUPPORTED, "window needs more shared memory than one CTA has");
+    const unsigned threads = 32u * (unsigned)(sh.rb / 2);
     ProfScope ps(H, TNLM_KERNEL_APPLY, st);
-    gj_apply_kernel<<<(unsigned)ctas, threads, smem, st>>>(R, g, u, out, wts);
+    switch (dp) {
+        case 16: gj_apply3_kernel<16><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+        case 8: gj_apply3_kernel<8><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+        default: gj_apply3_kernel<4><<<(unsigned)ctas, threads, sm, st>>>(R, g, u, out, wts); break;
+    }
     LAUNCHED(H);
     return TNLM_OK;
 }
@@ -1055,14 +968,10 @@ extern "C" int tnlm_set_option(tnlm_handle *H, const char *name, long long value
     if (n == "weight_cache_mb") H->opt_cache_mb = value;
     else if (n == "sweep_rb") { if ((ok = in(0, 64) && sweep_shape_known(H, (int)value, H->opt_nb))) H->opt_rb = (int)value; }
     else if (n == "sweep_nb") { if ((ok = in(0, 64) && sweep_shape_known(H, H->opt_rb, (int)value))) H->opt_nb = (int)value; }
-    else if (n == "apply_ns") { if ((ok = in(0, AP_NS_MAX))) H->opt_ns = (int)value; }
-    else if (n == "apply_kernel") { if ((ok = in(0, 2))) H->opt_apply = (int)value; }
     else if (n == "project_kernel") { if ((ok = in(-1, 1))) H->opt_project = (int)value; }
     else if (n == "apply_depth") { if ((ok = (value == 0 || value == 4 || value == 8 || value == 16))) H->opt_depth = (int)value; }
-    else if (n == "apply_wpc") { if ((ok = (value == 0 || in(2, 8)))) H->opt_wpc = (int)value; }
     else if (n == "project_interleave") { if ((ok = in(0, 1))) H->opt_project_il = (int)value; }
     else if (n == "project_block") { if ((ok = (value == 256 || value == 128 || value == 64))) H->opt_project_block = (int)value; }
-    else if (n == "project_group") { if ((ok = (value == 1 || value == 2 || value == 4))) H->opt_project_group = (int)value; }
     else if (n == "backproject_group") { if ((ok = (value == 1 || value == 2 || value == 4 || value == 8 || value == 16))) H->opt_backproject_group = (int)value; }
     else if (n == "apply_snake") { if ((ok = in(0, 1))) H->opt_snake = (int)value; }
     else if (n == "apply_resident_mb") { if ((ok = in(0, 1 << 20))) H->opt_resident_mb = value; }

@@ -184,8 +184,9 @@ def test_strip_and_gather_forward_projectors_are_bit_identical(T, cfg):
 
 
 def test_slice_groups_share_geometry_bit_identically(T):
-    # Slices of a batch have one geometry: the projectors serve groups of 8/4/2/1 slices per thread
-    # (options backproject_group, project_group).  S = 23 = 16 + 4 + 2 + 1 (= 8 + 8 + 4 + 2 + 1 ...) exercises every
+    # Slices of a batch have one geometry: the backprojector serves groups of 16/8/4/2/1 slices per thread (option
+    # backproject_group), the forward projector groups of four through interleaved copies (project_interleave) and the
+    # rest one per thread.  S = 23 = 16 + 4 + 2 + 1 (= 8 + 8 + 4 + 2 + 1 ...) exercises every
     # group size and the remainders; per slice the arithmetic is that of a single slice: bit-identical, and equal
     # to the oracle.
     torch, tn = T
@@ -199,8 +200,8 @@ def test_slice_groups_share_geometry_bit_identically(T):
     imgd, sinod, wd = dev(torch, img), dev(torch, sino), dev(torch, w)
     ref = {}
     # project_interleave: slices 0..19 through the interleaved copies (project_il_kernel, cgls_update_us_il), 20..22 not
-    for pg, bg, il in [(1, 1, 0), (2, 2, 0), (4, 4, 0), (4, 8, 1), (1, 16, 1), (2, 1, 1), (1, 16, 0)]:
-        tn.set_option(hd, "project_kernel", 0); tn.set_option(hd, "project_group", pg); tn.set_option(hd, "backproject_group", bg)
+    for bg, il in [(1, 0), (2, 0), (4, 0), (8, 1), (16, 1), (1, 1), (16, 0)]:
+        tn.set_option(hd, "project_kernel", 0); tn.set_option(hd, "backproject_group", bg)
         tn.set_option(hd, "project_interleave", il)
         po = torch.empty_like(sinod); bo = torch.empty_like(imgd); go = torch.empty_like(imgd)
         tn.project(hd, imgd, po); tn.backproject(hd, sinod, bo)
@@ -212,20 +213,20 @@ def test_slice_groups_share_geometry_bit_identically(T):
                 assert rel(bo[s].cpu().numpy(), oracle.backproject(og, sino[s], cfg.L, cfg.L)) < 2e-6
                 assert rel(go[s].cpu().numpy(), oracle.cgls_step(og, img[s], sino[s], w[s], 3)) < STEP_TOL
         else:
-            assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (pg, bg, il)
+            assert torch.equal(po, ref["p"]) and torch.equal(bo, ref["b"]) and torch.equal(go, ref["g"]), (bg, il)
     # project_block regroups only the ||q||^2 partial sums of the fused CGLS epilogue: P stays bit-identical, CGLS agrees to
     # rounding.  64 threads = two warps for the four slices of a group: every slice must still reach its reduction
     # (a slice that did not would keep its iterate, g = f).
-    for pg, il in [(4, 1), (4, 0), (1, 0)]:
-        tn.set_option(hd, "project_group", pg); tn.set_option(hd, "project_interleave", il)
+    for il in (1, 0):
+        tn.set_option(hd, "project_interleave", il)
         for bt in (64, 128, 256):
             tn.set_option(hd, "project_block", bt)
             po = torch.empty_like(sinod); go = torch.empty_like(imgd)
             tn.project(hd, imgd, po)
             tn.cgls_step(hd, imgd, sinod, wd, 3, go)
-            assert torch.equal(po, ref["p"]), (pg, il, bt)
+            assert torch.equal(po, ref["p"]), (il, bt)
             for s in range(S):
-                assert rel(go[s].cpu().numpy(), ref["g"][s].cpu().numpy()) < 1e-5, (pg, il, bt, s)
+                assert rel(go[s].cpu().numpy(), ref["g"][s].cpu().numpy()) < 1e-5, (il, bt, s)
 
 
 @pytest.mark.parametrize("B,V,L,sid", [(120, 16, 40, 45.0), (200, 9, 40, 45.0), (66, 40, 6, 14.6), (90, 12, 12, 15.0), (140, 7, 30, 27.5)],
@@ -553,11 +554,10 @@ def test_stored_weights_equal_recomputed_weights(T):
         assert np.abs(b.cpu().numpy() - want).max() < 1e-4 * np.abs(want).max()
 
 
-def test_both_stored_weight_sweep_kernels_agree(T):
-    # gj_apply3_kernel (default: one CTA per band, windows shared, per-warp cp.async rings), gj_apply2_kernel (option
-    # apply_kernel = 1: persistent warp tasks, cp.async rings, every ring depth and CTA size the cost model
-    # may pick) and gj_apply_kernel (option apply_kernel = 0: one CTA per band, TMA ring) read the same stored layout
-    # and accumulate in the same order: bit-identical results; both match the oracle.
+def test_stored_weight_sweep_is_bit_identical_over_its_launch_options(T):
+    # gj_apply3_kernel (opt-in stored weights: one CTA per band, windows shared, per-warp cp.async rings): the ring depth,
+    # the order in which successive sweeps take the bands (snake) and the L2 residency hints change where bytes come
+    # from and when, not one bit of the result; the result matches the oracle.
     torch, tn = T
     for (N, ny, nx, W, d, h, mu, m2) in [(3, 70, 132, 11, 5, 0.008, 0.3, 4), (2, 45, 300, 15, 7, 0.006, 0.2, 3), (4, 33, 50, 3, 3, 0.01, 0.4, 3)]:
         g = noisy_stack(N, ny, nx, seed=91)
@@ -565,29 +565,15 @@ def test_both_stored_weight_sweep_kernels_agree(T):
         hd = tn.create(None, nx, ny, N, W, d, h, mu)
         tn.set_option(hd, "weight_cache_mb", 16384)
         ref = torch.empty_like(gd)
-        tn.set_option(hd, "apply_kernel", 0)
         tn.regularize_step(hd, gd, m2, ref)
         assert rel(ref.cpu().numpy(), oracle.regularize_step(g, W, d, h, mu, m2)) < STEP_TOL
-        for depth in (0, 4, 16):                 # gj_apply3_kernel: one CTA per band, both windows shared by its warps
-            tn.set_option(hd, "apply_kernel", 2); tn.set_option(hd, "apply_depth", depth)
-            out = torch.empty_like(gd)
-            tn.regularize_step(hd, gd, m2, out)
-            assert torch.equal(out, ref), (W, "apply3", depth)
-        tn.set_option(hd, "apply_kernel", 1)
-        for depth, wpc in [(0, 0), (4, 2), (8, 3), (16, 8), (8, 6)]:
-            tn.set_option(hd, "apply_depth", depth); tn.set_option(hd, "apply_wpc", wpc)
-            out = torch.empty_like(gd)
-            tn.regularize_step(hd, gd, m2, out)
-            assert torch.equal(out, ref), (W, depth, wpc)
-        # task order (snake over the sweeps) and L2 residency hints change where bytes come from, not one bit
-        tn.set_option(hd, "apply_depth", 0); tn.set_option(hd, "apply_wpc", 0)
-        for kern in (1, 2):
-            tn.set_option(hd, "apply_kernel", kern)
+        for depth in (4, 8, 16, 0):
+            tn.set_option(hd, "apply_depth", depth)
             for snake, mb in [(0, 0), (1, 0), (0, 1), (1, 1), (1, 4096)]:
                 tn.set_option(hd, "apply_snake", snake); tn.set_option(hd, "apply_resident_mb", mb)
                 out = torch.empty_like(gd)
                 tn.regularize_step(hd, gd, m2, out)
-                assert torch.equal(out, ref), (W, kern, snake, mb)
+                assert torch.equal(out, ref), (W, depth, snake, mb)
 
 
 def test_regularize_multi_slice_equals_per_slice(T):
@@ -626,7 +612,7 @@ def test_config2_full_size_on_sampled_pixels(T):
 
 def test_config2_headline_call_ten_sweeps_matches_oracle(T):
     # The call bench.py times: tnlm_regularize_step(m2 = 10) on BASELINE config 2, i.e. one
-    # gj_sweep_kernel<.,.,true> launch and nine gj_apply_kernel launches reading bf16 stored weights,
+    # gj_sweep_kernel<.,.,true> launch and nine gj_apply3_kernel launches reading bf16 stored weights (opt-in),
     # against the oracle's ten fp64 sweeps, every pixel; and the same with the weights recomputed in
     # fp32 every sweep (weight_cache_mb = 0).  PAPER.md:L147-L158, L162.
     torch, tn = T
